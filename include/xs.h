@@ -1,0 +1,172 @@
+/*
+ * xs.h -- C ABI of the B200 quasi-greedy clone-sweep library (libxs_b200.so).
+ *
+ * What the library computes (PAPER.md = text of arXiv 2102.09510; line numbers cited):
+ *   the quasi-greedy (QG) local search of PAPER.md L65-L71 / L101 run on many "clones"
+ *   (L73-L85) of the diluted 3-spin model H = -sum_{(i,j,k) in E} J_ijk s_i s_j s_k on a
+ *   random 3-regular 3-uniform hypergraph (L41 Eq.(1)), clones bit-packed as multi-spin
+ *   coded words (L87), swept set by set over independent sets of spins (L277-L289), with
+ *   the exact sweep of the first ground-state hit recorded per clone (L293) and the run's
+ *   time-to-solution TTS = min over clones (L111).  DESIGN.md lists every reading taken
+ *   where the paper is silent (noise granularity, Philox counters, order, stop rule).
+ *
+ * Conventions
+ *   - Everything is integer / Boolean; there is no floating point on the path except in
+ *     the small host statistics of xs_tts_stats.
+ *   - "dev" pointers are CUDA device pointers owned by the caller (e.g. torch tensors'
+ *     data_ptr()); "host" pointers are ordinary host memory.  The library never allocates
+ *     device memory and never creates streams.  `cuda_stream` is a cudaStream_t passed as
+ *     void* (NULL = the legacy default stream).
+ *   - State layout: x[inst][i][w], uint64, i = spin 0..N-1, w = word 0..W-1; bit b of word w
+ *     is clone c = 64 w + b; bit value 1 <=> s_i = -1.  (SURVEY.md section 8(a).)
+ *   - Sweep index t is 1-based and global per instance: a call continues where the previous
+ *     one stopped.  first_hit[inst][c] = t of the first sweep after which clone c has
+ *     E = -N (0 if the initial state already has; XS_NO_HIT = never so far).
+ *   - Every call returns 0 (XS_OK) or a negative error code; nothing throws or aborts across
+ *     the ABI; xs_last_error() returns a thread-local description of the last failure.
+ *   - All calls that take a stream only enqueue work on it; xs_tts also synchronises it.
+ *     xs_create_instance* additionally block the host until the table uploads are done.
+ */
+#ifndef XS_H_
+#define XS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define XS_OK       0
+#define XS_EINVAL  -1   /* null pointer, bad shape (N < 3, W = 0, n_instances = 0), bad array contents */
+#define XS_ENOMEM  -2   /* caller's workspace too small / host allocation failed                        */
+#define XS_ECUDA   -3   /* a CUDA runtime call or kernel launch failed                                   */
+#define XS_ESTATE  -4   /* call order / handle misuse (e.g. sweep counter would overflow)                */
+
+#define XS_NO_HIT  0xFFFFFFFFu
+
+/* xs_params.flags */
+#define XS_FLAG_GAUGE        1u  /* planted gauge: J_t = tau_i tau_j tau_k (BASELINE.json configs);
+                                    off => J = +1, the paper's ferromagnet (L43)                        */
+#define XS_FLAG_NO_SKIP      2u  /* keep sweeping instances that already have a solved clone
+                                    (config 2: fixed sweep count).  Default: an instance whose solved
+                                    flag is set at call entry is skipped (L129/L293 stop rule)          */
+#define XS_FLAG_STREAMING    4u  /* force the streaming (global-memory) regime even if a tile fits
+                                    on chip; the regimes are bit-identical (tests use this)             */
+
+/* w1 = 0.055 (L101) as a 32-bit threshold: flip a k=1 spin iff u32 < floor(0.055 * 2^32). */
+#define XS_W1_THRESHOLD_DEFAULT 236223201u
+
+typedef struct xs_batch xs_batch;       /* opaque: >= 1 instances of equal N and W */
+
+typedef struct {
+    uint32_t n_spins;        /* N: spins = triplets per instance (L43), >= 3                     */
+    uint32_t n_words;        /* W: uint64 words per spin; 64 W clones per instance (L87), >= 1   */
+    uint32_t n_instances;    /* >= 1                                                             */
+    uint32_t set_cap;        /* cap on independent-set size; 0 = uncapped (paper: 32, L279)      */
+    uint32_t w1_threshold;   /* see XS_W1_THRESHOLD_DEFAULT                                      */
+    uint32_t flags;          /* XS_FLAG_*                                                        */
+} xs_params;
+
+typedef struct {
+    uint32_t solved;         /* 1 iff some clone of the instance has first_hit != XS_NO_HIT      */
+    uint32_t tts_sweeps;     /* min_c first_hit (L111), XS_NO_HIT if not solved                  */
+    uint32_t clone;          /* smallest clone index attaining the minimum, XS_NO_HIT if none    */
+    uint32_t _pad;
+    uint64_t sweeps_done;    /* sweeps performed on this instance so far                         */
+} xs_tts_rec;
+
+/* Host-side description of the launch geometry chosen for a batch (for bench / roofline). */
+typedef struct {
+    uint32_t regime;         /* 0 = on-chip tile kernel, 1 = streaming kernel                    */
+    uint32_t tile_words;     /* T: uint64 columns per CTA tile (on-chip), W (streaming)          */
+    uint32_t threads;        /* threads per CTA                                                  */
+    uint32_t ctas;           /* CTAs per xs_run_sweeps launch                                    */
+    uint32_t smem_bytes;     /* dynamic shared memory per CTA                                    */
+    uint32_t batch_sweeps;   /* sweeps between ground-state checks inside the kernel             */
+    uint32_t n_sets_max;     /* largest number of independent sets over the instances            */
+    uint32_t _pad;
+} xs_layout;
+
+/* Bytes of device workspace a batch with these parameters needs (state, first-hit table,
+ * graph tables, per-instance records).  Host call, no CUDA work. */
+int xs_workspace_bytes(const xs_params* p, size_t* device_bytes);
+
+/* a-1 + a-2 of DESIGN.md.  Builds n_instances instances on the host from graph_seeds[inst]
+ * (configuration model with rejection, planted gauge, adjacency, greedy independent sets;
+ * DESIGN.md section "Readings"), uploads the tables into dev_ws (caller-owned, at least
+ * xs_workspace_bytes, 256-byte aligned), and enqueues the init kernel that writes the random
+ * initial clone states from Philox(run_seeds[inst]) (L77) and marks clones that start in a
+ * ground state.  graph_seeds / run_seeds: host arrays [n_instances].  The handle owns only
+ * host metadata; free it with xs_destroy.  The workspace must outlive the handle. */
+int xs_create_instance(xs_batch** out, const xs_params* p, const uint64_t* graph_seeds,
+                       const uint64_t* run_seeds, void* dev_ws, size_t ws_bytes,
+                       void* cuda_stream);
+
+/* Same, but the instances are given explicitly (host arrays):
+ *   tri      [inst][N][3]  spin indices of each triplet (each spin in exactly 3, distinct in a triplet)
+ *   jbit     [inst][N]     1 <=> J_t = -1
+ *   order    [inst][N]     update order: concatenation of the independent sets (L289)
+ *   set_size [inst][n_sets_max] sizes of the sets, zero padded; n_sets[inst] = number used.
+ * Every set must be an anti-clique (L277); violations give XS_EINVAL. */
+int xs_create_instance_from_arrays(xs_batch** out, const xs_params* p, const uint32_t* tri,
+                                   const uint8_t* jbit, const uint32_t* order,
+                                   const uint32_t* set_size, const uint32_t* n_sets,
+                                   uint32_t n_sets_max, const uint64_t* run_seeds,
+                                   void* dev_ws, size_t ws_bytes, void* cuda_stream);
+
+/* a-3 .. a-10 (+ the termination part of a-11).  Advances every instance that is not
+ * skipped (see XS_FLAG_NO_SKIP) by exactly n_sweeps sweeps (L65-L67 rule, L87 one random
+ * number per word, L277 set by set), keeps first_hit exact, then refreshes the
+ * per-instance solved / TTS records on the device.  Asynchronous on cuda_stream. */
+int xs_run_sweeps(xs_batch* b, uint64_t n_sweeps, void* cuda_stream);
+
+/* a-11.  E_c = -sum_t J_t s_i s_j s_k (L41) for every clone: dev_out [inst][64 W] int32. */
+int xs_energy(xs_batch* b, int32_t* dev_out, void* cuda_stream);
+
+/* a-11/a-12.  Copies the per-instance records to host_out [n_instances] and synchronises
+ * cuda_stream. */
+int xs_tts(xs_batch* b, xs_tts_rec* host_out, void* cuda_stream);
+
+/* State access (device to device, async).  xs_set_spins also recomputes first_hit from
+ * scratch for the new state (clones in a ground state get the current sweep count) and
+ * clears the solved flags accordingly; the sweep counters are unchanged. */
+int xs_get_spins(xs_batch* b, uint64_t* dev_out /* [inst][N][W] */, void* cuda_stream);
+int xs_set_spins(xs_batch* b, const uint64_t* dev_in /* [inst][N][W] */, void* cuda_stream);
+int xs_get_first_hit(xs_batch* b, uint32_t* dev_out /* [inst][64 W] */, void* cuda_stream);
+
+/* Host copies of instance `inst`'s graph: tri [N][3], jbit [N], order [N], set_size [N]
+ * (first *n_sets entries valid).  Any pointer may be NULL.  No CUDA work. */
+int xs_get_graph(const xs_batch* b, uint32_t inst, uint32_t* tri, uint8_t* jbit,
+                 uint32_t* order, uint32_t* set_size, uint32_t* n_sets);
+
+/* a-1 alone, host only (no CUDA work): builds one instance from graph_seed exactly as
+ * xs_create_instance does and writes tri [N][3], jbit [N], order [N], set_size [N] (first
+ * *n_sets entries valid), *attempt = index of the accepted configuration-model attempt.
+ * Any output pointer may be NULL.  flags: only XS_FLAG_GAUGE is looked at. */
+int xs_generate_graph(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uint32_t set_cap,
+                      uint32_t* tri, uint8_t* jbit, uint32_t* order, uint32_t* set_size,
+                      uint32_t* n_sets, int32_t* attempt);
+
+/* Launch geometry the library chose for this batch.  No CUDA work. */
+int xs_get_layout(const xs_batch* b, xs_layout* out);
+
+/* a-12.  TTS statistics "as the paper defines" (L103-L149) over n_runs runs of one instance
+ * with sweep cap t_max: tts[r] = TTS in sweeps or XS_NO_HIT (censored).  Host only.
+ *   out[0] = n (solved runs)                     out[1] = T_tot = sum_solved tts + (n_runs-n) t_max
+ *   out[2] = tau_hat = T_tot / n (L139-L147: maximum of the posterior's likelihood; inf if n=0)
+ *   out[3..5] = model TTS_50/90/99 = -ln(1-p) tau_hat (L117, L123)
+ *   out[6..8] = empirical TTS_50/90/99: the ceil(p n_runs)-th smallest value, censored runs
+ *               counting as +inf (L103, L115)
+ *   out[9..11] = 16 / 50 / 84 % quantiles of the posterior of tau, inverse-gamma(shape n,
+ *               scale T_tot) (L145); for n = 0, out[9] = T_tot / ln 20 (95 % lower bound), rest inf. */
+int xs_tts_stats(const uint32_t* tts, uint32_t n_runs, uint64_t t_max, double* out /* [12] */);
+
+int xs_destroy(xs_batch* b);
+
+const char* xs_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XS_H_ */

@@ -1,0 +1,105 @@
+// xs_internal.h -- declarations shared by the translation units of libxs_b200.so.
+// Product code: shares nothing with oracle/ (own Philox, own generator).
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/xs.h"
+
+namespace xs {
+
+// Domain tags in Philox counter word 3.
+enum : uint32_t { TAG_GRAPH = 1, TAG_GAUGE = 2, TAG_INIT = 3, TAG_SWEEP = 4 };
+
+// ---- host-side instance (a-1) -------------------------------------------------------------
+struct HostGraph {
+    uint32_t n = 0;
+    std::vector<uint32_t> tri;       // [N][3]
+    std::vector<uint8_t> jbit;       // [N]
+    std::vector<uint32_t> nbr;       // [N][6]  partners of spin i in its clauses (ascending clause id)
+    std::vector<uint32_t> cls;       // [N][3]  clause ids of spin i
+    std::vector<uint32_t> order;     // [N]
+    std::vector<uint32_t> set_start; // [n_sets + 1]
+    int attempt = -1;                // accepted attempt of the configuration model
+};
+
+void philox4x32_10_host(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+// Build from seeds (configuration model with rejection, gauge, adjacency, greedy sets).
+// Returns false and sets err on failure.
+bool build_graph_from_seed(uint32_t n, uint64_t graph_seed, bool gauge, uint32_t set_cap,
+                           HostGraph& g, std::string& err);
+// Build from explicit arrays; validates 3-regularity and that every set is an anti-clique.
+bool build_graph_from_arrays(uint32_t n, const uint32_t* tri, const uint8_t* jbit,
+                             const uint32_t* order, const uint32_t* set_size, uint32_t n_sets,
+                             HostGraph& g, std::string& err);
+
+// ---- device tables --------------------------------------------------------------------------
+// Adjacency record of the spin at position p of the update order (32 bytes, 2 x 16 B loads).
+struct alignas(16) AdjRec {
+    uint32_t nbr[6];   // spin indices: (nbr[2r], nbr[2r+1]) = partners in clause r
+    uint32_t self;     // spin index of this position
+    uint32_t jbits;    // bit r = coupling bit of clause r (1 <=> J = -1)
+};
+// Clause record for the energy / ground-state kernels (16 bytes).
+struct alignas(16) ClauseRec {
+    uint32_t i, j, k, jbit;
+};
+
+// Device workspace carved out of the caller's buffer.
+struct DevLayout {
+    size_t off_x = 0, off_first_hit = 0, off_adj = 0, off_clause = 0, off_set_start = 0,
+           off_rec = 0, off_seed = 0, off_det = 0, off_nsets = 0, total = 0;
+};
+DevLayout make_layout(const xs_params& p);
+
+struct DevPtrs {
+    uint64_t* x;           // [I][N][W]
+    uint32_t* first_hit;   // [I][64W]
+    AdjRec* adj;           // [I][N]   (order position)
+    ClauseRec* clause;     // [I][N]
+    uint32_t* set_start;   // [I][N+1]
+    xs_tts_rec* rec;       // [I]
+    uint64_t* run_seed;    // [I]
+    uint64_t* det;         // [I][W]   scratch: OR of unsatisfied-clause words
+    uint32_t* n_sets;      // [I]
+};
+
+struct TileGeom {
+    uint32_t regime = 0;       // 0 on-chip, 1 streaming
+    uint32_t T = 0;            // uint64 columns per tile
+    uint32_t CW = 0;           // words per lane (1 or 2)
+    uint32_t threads = 0;
+    uint32_t ctas = 0;
+    uint32_t smem = 0;
+    uint32_t batch = 0;        // sweeps between in-kernel ground-state checks
+    uint32_t rb = 0;           // sweeps of random bytes produced at a time
+    uint32_t variant = 0;
+};
+
+}  // namespace xs
+
+struct xs_batch {
+    xs_params p{};
+    std::vector<xs::HostGraph> graphs;
+    std::vector<uint64_t> run_seeds;
+    xs::DevLayout lay;
+    xs::DevPtrs d{};
+    xs::TileGeom geom;
+    uint32_t n_sets_max = 0;
+    uint32_t max_set_size = 0;
+    uint64_t sweeps_issued = 0;   // upper bound on any instance's sweep counter (overflow guard)
+    void* ws = nullptr;
+};
+
+namespace xs {
+// kernels (xs_kernels.cu); every launcher returns a cudaError_t as int.
+int launch_init(const xs_batch& b, void* stream);
+int launch_mark(const xs_batch& b, bool reset_first_hit, void* stream);   // ground-state marking at current t
+int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream);
+int launch_finalize(const xs_batch& b, uint32_t n_sweeps, void* stream);
+int launch_energy(const xs_batch& b, int32_t* dev_out, void* stream);
+bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err);
+}  // namespace xs

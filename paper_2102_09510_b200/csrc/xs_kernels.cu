@@ -1,0 +1,835 @@
+// xs_kernels.cu -- the CUDA path of the quasi-greedy clone sweep (sm_100a).
+//
+// Kernels:
+//   k_init          a-2   random initial clone words from Philox(INIT)
+//   k_sweep_tile    a-3..a-10  on-chip regime: a CTA owns (instance, T word columns), keeps the
+//                   tile in shared memory for all sweeps of the call               (L293-L295)
+//   k_stream_set    a-4..a-9   streaming regime: one launch per independent set, state in HBM/L2
+//   k_unsat_or / k_mark / k_stream_commit   a-9/a-11  ground-state detection, first-hit table
+//   k_energy_*      a-11  per-clone energies                                       (L41 Eq.(1))
+//   k_finalize      a-11/a-12  per-instance min first-hit, solved flag, sweep counter (L111)
+//
+// The update itself (a-4..a-7), per 32 clones, all Boolean (L87 "multi-spin coding"):
+//   w_r = x_a ^ x_b ^ Jmask_r            r = 0,1,2      clause fields without the spin itself
+//   M = maj(w_0,w_1,w_2), P = w_0^w_1^w_2               bit-sliced adder of the three
+//   unsatisfied-clause count of the spin: k = 2 (M^x) + (P^x) by self-duality of maj / parity
+//   QG rule w = (0, w1, 1, 1) (L65-L67, L101): flip = (M^x) | ((P^x) & R)
+//     R = 0  -> x_new = M ;  R = ~0 -> x_new = maj(M, P, ~x)
+//   R = all-ones iff the word's 32-bit Philox output is below w1_threshold (L87: one random
+//   number per word of clones).
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+
+#include "xs_internal.h"
+
+namespace xs {
+
+// ------------------------------------------------------------------------------------------
+// device helpers
+// ------------------------------------------------------------------------------------------
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return d;
+}
+// LUT index = a*4 + b*2 + c
+constexpr int LUT_XOR3 = 0x96;
+constexpr int LUT_MAJ = 0xE8;
+constexpr int LUT_MAJ_NOTC = 0xD4;   // maj(a, b, ~c)
+constexpr int LUT_SEL = 0xCA;        // a ? b : c
+constexpr int LUT_NZ = 0x7E;         // (a^c)|(b^c): not all equal
+constexpr int LUT_OR3 = 0xFE;
+
+// Philox4x32-10 (Salmon et al., SC'11).  ctr = (c0,c1,c2,c3), key = (k0,k1).
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t o[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0);
+        const uint32_t l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2);
+        const uint32_t l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0;
+        c2 = h0 ^ c3 ^ k1;
+        c1 = l1;
+        c3 = l0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
+}
+
+// One QG update of 32 clones.  a*/b* partner words, j* coupling masks, x own word, R noise mask.
+__device__ __forceinline__ uint32_t qg_update(uint32_t a0, uint32_t b0, uint32_t j0, uint32_t a1,
+                                              uint32_t b1, uint32_t j1, uint32_t a2, uint32_t b2,
+                                              uint32_t j2, uint32_t x, uint32_t R)
+{
+    const uint32_t w0 = lop3<LUT_XOR3>(a0, b0, j0);
+    const uint32_t w1 = lop3<LUT_XOR3>(a1, b1, j1);
+    const uint32_t w2 = lop3<LUT_XOR3>(a2, b2, j2);
+    const uint32_t M = lop3<LUT_MAJ>(w0, w1, w2);
+    const uint32_t P = lop3<LUT_XOR3>(w0, w1, w2);
+    const uint32_t f = lop3<LUT_MAJ_NOTC>(M, P, x);
+    return lop3<LUT_SEL>(R, f, M);
+}
+// Bits set where the spin has k != 0 unsatisfied clauses.
+__device__ __forceinline__ uint32_t qg_nonzero_k(uint32_t a0, uint32_t b0, uint32_t j0, uint32_t a1,
+                                                 uint32_t b1, uint32_t j1, uint32_t a2, uint32_t b2,
+                                                 uint32_t j2, uint32_t x)
+{
+    const uint32_t w0 = lop3<LUT_XOR3>(a0, b0, j0);
+    const uint32_t w1 = lop3<LUT_XOR3>(a1, b1, j1);
+    const uint32_t w2 = lop3<LUT_XOR3>(a2, b2, j2);
+    const uint32_t M = lop3<LUT_MAJ>(w0, w1, w2);
+    const uint32_t P = lop3<LUT_XOR3>(w0, w1, w2);
+    return lop3<LUT_NZ>(M, P, x);
+}
+
+// CW uint64 words handled by one lane, as 2*CW uint32.
+template <int CW> struct Vec;
+template <> struct Vec<1> { uint2 v; };
+template <> struct Vec<2> { uint4 v; };
+
+template <int CW> __device__ __forceinline__ void vload(const void* p, uint32_t (&o)[2 * CW]);
+template <> __device__ __forceinline__ void vload<1>(const void* p, uint32_t (&o)[2])
+{
+    const uint2 t = *reinterpret_cast<const uint2*>(p);
+    o[0] = t.x; o[1] = t.y;
+}
+template <> __device__ __forceinline__ void vload<2>(const void* p, uint32_t (&o)[4])
+{
+    const uint4 t = *reinterpret_cast<const uint4*>(p);
+    o[0] = t.x; o[1] = t.y; o[2] = t.z; o[3] = t.w;
+}
+template <int CW> __device__ __forceinline__ void vstore(void* p, const uint32_t (&o)[2 * CW]);
+template <> __device__ __forceinline__ void vstore<1>(void* p, const uint32_t (&o)[2])
+{
+    *reinterpret_cast<uint2*>(p) = make_uint2(o[0], o[1]);
+}
+template <> __device__ __forceinline__ void vstore<2>(void* p, const uint32_t (&o)[4])
+{
+    *reinterpret_cast<uint4*>(p) = make_uint4(o[0], o[1], o[2], o[3]);
+}
+
+// ------------------------------------------------------------------------------------------
+// a-2: initial state.  word(i,w) = o0 | o1 << 32 of Philox(ctr = (i, w, 0, INIT), key = run seed)
+// ------------------------------------------------------------------------------------------
+__global__ void k_init(DevPtrs d, uint32_t N, uint32_t W, uint32_t I)
+{
+    const uint64_t total = (uint64_t)I * N * W;
+    for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t w = (uint32_t)(e % W);
+        const uint32_t i = (uint32_t)((e / W) % N);
+        const uint32_t inst = (uint32_t)(e / ((uint64_t)W * N));
+        const uint64_t seed = d.run_seed[inst];
+        uint32_t o[4];
+        philox4x32_10(i, w, 0u, TAG_INIT, (uint32_t)seed, (uint32_t)(seed >> 32), o);
+        d.x[e] = (uint64_t)o[0] | ((uint64_t)o[1] << 32);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a-9 / a-11: ground-state detection from global memory.
+// det[inst][w] |= OR over clauses of (x_i ^ x_j ^ x_k ^ Jmask): bit c set <=> clone c has an
+// unsatisfied clause <=> E_c > -N (L41: each of the N terms is >= -1).
+// grid = (clause chunks, I); a thread owns words w = tid, tid + blockDim, ...
+// ------------------------------------------------------------------------------------------
+constexpr uint32_t DET_CHUNK = 64;
+
+__global__ void k_unsat_or(DevPtrs d, uint32_t N, uint32_t W, uint64_t* det)
+{
+    const uint32_t inst = blockIdx.y;
+    const uint32_t c0 = blockIdx.x * DET_CHUNK;
+    const uint32_t c1 = min(c0 + DET_CHUNK, N);
+    const ClauseRec* cl = d.clause + (size_t)inst * N;
+    const uint64_t* x = d.x + (size_t)inst * N * W;
+    for (uint32_t w = threadIdx.x; w < W; w += blockDim.x) {
+        uint64_t acc = 0;
+        for (uint32_t c = c0; c < c1; ++c) {
+            const ClauseRec r = cl[c];
+            const uint64_t jm = r.jbit ? ~0ull : 0ull;
+            acc |= x[(size_t)r.i * W + w] ^ x[(size_t)r.j * W + w] ^ x[(size_t)r.k * W + w] ^ jm;
+        }
+        if (acc) atomicOr(reinterpret_cast<unsigned long long*>(det + (size_t)inst * W + w), acc);
+    }
+}
+
+// first_hit[clone] = sweeps_done[inst] for clones whose det bit is clear.  reset != 0: rewrite
+// the whole table (XS_NO_HIT elsewhere); reset == 0: only fill entries that are XS_NO_HIT.
+__global__ void k_mark(DevPtrs d, uint32_t W, uint32_t I, const uint64_t* det, int reset,
+                       uint32_t t_add)
+{
+    const uint64_t total = (uint64_t)I * W * 64;
+    for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t inst = (uint32_t)(e / ((uint64_t)W * 64));
+        const uint64_t word = det[e >> 6];
+        const bool solved = ((word >> (e & 63)) & 1ull) == 0;
+        const uint32_t t_now = (uint32_t)d.rec[inst].sweeps_done + t_add;
+        if (reset)
+            d.first_hit[e] = solved ? t_now : XS_NO_HIT;
+        else if (solved && d.first_hit[e] == XS_NO_HIT)
+            d.first_hit[e] = t_now;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a-11: energies.  E_c = -N + 2 U_c, U_c = number of unsatisfied clauses of clone c.
+// Bit-sliced vertical counters per thread (multi-spin coding of the count, L87), then expanded.
+// grid = (W, I, clause chunks)
+// ------------------------------------------------------------------------------------------
+constexpr uint32_t EN_THREADS = 128;
+constexpr uint32_t EN_CHUNK = 8192;
+
+__global__ void k_energy_fill(int32_t* out, uint64_t total, int32_t value)
+{
+    for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (uint64_t)gridDim.x * blockDim.x)
+        out[e] = value;
+}
+
+__global__ void __launch_bounds__(EN_THREADS) k_energy_acc(DevPtrs d, uint32_t N, uint32_t W,
+                                                          int32_t* out)
+{
+    __shared__ int cnt[64];
+    const uint32_t w = blockIdx.x, inst = blockIdx.y;
+    const uint32_t c0 = blockIdx.z * EN_CHUNK;
+    const uint32_t c1 = min(c0 + EN_CHUNK, N);
+    if (threadIdx.x < 64) cnt[threadIdx.x] = 0;
+    __syncthreads();
+    const ClauseRec* cl = d.clause + (size_t)inst * N;
+    const uint64_t* x = d.x + (size_t)inst * N * W;
+    // planes[p] holds bit p of the per-clone count; EN_CHUNK / EN_THREADS = 64 clauses per
+    // thread at most -> 7 planes.
+    uint64_t planes[7] = {0, 0, 0, 0, 0, 0, 0};
+    for (uint32_t c = c0 + threadIdx.x; c < c1; c += EN_THREADS) {
+        const ClauseRec r = cl[c];
+        uint64_t carry = x[(size_t)r.i * W + w] ^ x[(size_t)r.j * W + w] ^ x[(size_t)r.k * W + w] ^
+                         (r.jbit ? ~0ull : 0ull);
+#pragma unroll
+        for (int p = 0; p < 7; ++p) {
+            const uint64_t s = planes[p] ^ carry;
+            carry &= planes[p];
+            planes[p] = s;
+        }
+    }
+    for (int b = 0; b < 64; ++b) {
+        int v = 0;
+#pragma unroll
+        for (int p = 0; p < 7; ++p) v |= (int)((planes[p] >> b) & 1ull) << p;
+        if (v) atomicAdd(&cnt[b], v);
+    }
+    __syncthreads();
+    if (threadIdx.x < 64 && cnt[threadIdx.x])
+        atomicAdd(out + ((size_t)inst * W + w) * 64 + threadIdx.x, 2 * cnt[threadIdx.x]);
+}
+
+// ------------------------------------------------------------------------------------------
+// a-11 / a-12: per-instance record.  TTS = min_c first_hit (L111); smallest clone on ties.
+// One CTA per instance.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_finalize(DevPtrs d, uint32_t W, uint32_t n_sweeps,
+                                                  uint32_t flags)
+{
+    __shared__ unsigned long long best[8];
+    const uint32_t inst = blockIdx.x;
+    const uint32_t C = 64 * W;
+    const uint32_t* fh = d.first_hit + (size_t)inst * C;
+    unsigned long long m = ~0ull;
+    for (uint32_t c = threadIdx.x; c < C; c += blockDim.x) {
+        const unsigned long long v = ((unsigned long long)fh[c] << 32) | c;
+        m = v < m ? v : m;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long v = __shfl_xor_sync(0xFFFFFFFFu, m, o);
+        m = v < m ? v : m;
+    }
+    if ((threadIdx.x & 31) == 0) best[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (uint32_t q = 1; q < blockDim.x / 32; ++q) m = best[q] < m ? best[q] : m;
+        xs_tts_rec r = d.rec[inst];
+        const bool skipped = r.solved && !(flags & XS_FLAG_NO_SKIP);
+        if (!skipped) r.sweeps_done += n_sweeps;
+        const uint32_t t = (uint32_t)(m >> 32);
+        r.solved = (t != XS_NO_HIT) ? 1u : 0u;
+        r.tts_sweeps = t;
+        r.clone = (t != XS_NO_HIT) ? (uint32_t)m : XS_NO_HIT;
+        r._pad = 0;
+        d.rec[inst] = r;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a-3 .. a-10: on-chip regime.
+//
+// A CTA owns tile (inst, word columns [w0, w0 + T)) for the whole call: the N x T uint64 tile
+// lives in shared memory as rows x[i][0..T) (copy in, ~100 sweeps, copy
+// out).  Unlike the paper's lanes <-> spins mapping (L277), LANES <-> CLONE WORDS of one spin
+// row: the LPS = T / CW lanes that share a spin read the same partner rows, so every gather is
+// a contiguous row read and the partner indices are shared by the lane group.  Different lane
+// groups ("slots") take different spins of the current independent set; __syncthreads() after
+// each set (L277).
+//
+// Noise: the Philox outputs of a whole chunk of sweeps are turned into one byte per
+// (sweep, position, word) (0xFF <=> u32 < w1_threshold) by all threads in a produce phase, so
+// that each Philox call (4 words) is computed once and off the update's critical path.
+//
+// Ground-state detection (a-9) without touching the hot loop: every `batch` sweeps the CTA
+// runs a detection pass (k != 0 accumulate over all spins).  If a clone not yet in the
+// first-hit table is solved, the batch is replayed from the copy of the tile in global memory
+// (written at every batch boundary) with a detection pass after every sweep, which yields the
+// exact first-hit sweep (L293); counter-based noise makes the replay bit-identical.
+// ------------------------------------------------------------------------------------------
+struct TileArgs {
+    DevPtrs d;
+    uint32_t N, W, T, n_sweeps, thr, flags, batch, rb;
+    uint32_t off_rec, off_rbuf, off_sets, off_misc;   // byte offsets in dynamic shared memory
+};
+
+template <int CW>
+struct TileCtx {
+    unsigned char* state;     // [N][T] uint64
+    const uint4* rec;         // [N][3]
+    unsigned char* rbuf;      // [rb][N][T] bytes
+    const uint32_t* sets;     // [n_sets + 1]
+    uint32_t* det32;          // [2T]
+    uint32_t* known32;        // [2T]
+    uint32_t* flag;
+    uint32_t N, T, n_sets, slot, n_slots, joff /* byte offset of this lane's words in a row */,
+        jw /* first local word of this lane */;
+};
+
+template <int CW>
+__device__ __forceinline__ void tile_gather(const TileCtx<CW>& c, uint32_t p, uint32_t (&a)[3][2 * CW],
+                                            uint32_t (&b)[3][2 * CW], uint32_t (&x)[2 * CW],
+                                            uint32_t (&jm)[3], uint32_t& self_off)
+{
+    const uint4 r0 = c.rec[3 * p], r1 = c.rec[3 * p + 1], r2 = c.rec[3 * p + 2];
+    vload<CW>(c.state + r0.x + c.joff, a[0]);
+    vload<CW>(c.state + r0.y + c.joff, b[0]);
+    vload<CW>(c.state + r0.z + c.joff, a[1]);
+    vload<CW>(c.state + r0.w + c.joff, b[1]);
+    vload<CW>(c.state + r1.x + c.joff, a[2]);
+    vload<CW>(c.state + r1.y + c.joff, b[2]);
+    vload<CW>(c.state + r1.z + c.joff, x);
+    self_off = r1.z;
+    jm[0] = r2.x; jm[1] = r2.y; jm[2] = r2.z;
+}
+
+// one sweep over all sets, sweep slot `rs` of the random-byte ring
+template <int CW>
+__device__ __forceinline__ void tile_sweep(const TileCtx<CW>& c, uint32_t rs)
+{
+    const unsigned char* rb = c.rbuf + (size_t)rs * c.N * c.T + c.jw;
+    for (uint32_t s = 0; s < c.n_sets; ++s) {
+        const uint32_t p1 = c.sets[s + 1];
+        for (uint32_t p = c.sets[s] + c.slot; p < p1; p += c.n_slots) {
+            uint32_t a[3][2 * CW], b[3][2 * CW], x[2 * CW], jm[3], self_off;
+            tile_gather<CW>(c, p, a, b, x, jm, self_off);
+            uint32_t R[CW];
+            if (CW == 2) {
+                const uint32_t two = *reinterpret_cast<const unsigned short*>(rb + (size_t)p * c.T);
+                R[0] = (uint32_t)(int32_t)(int8_t)(two & 0xFF);
+                R[CW - 1] = (uint32_t)(int32_t)(int8_t)(two >> 8);
+            } else {
+                R[0] = (uint32_t)(int32_t)(int8_t)rb[(size_t)p * c.T];
+            }
+            uint32_t xn[2 * CW];
+#pragma unroll
+            for (int h = 0; h < 2 * CW; ++h)
+                xn[h] = qg_update(a[0][h], b[0][h], jm[0], a[1][h], b[1][h], jm[1], a[2][h], b[2][h],
+                                  jm[2], x[h], R[h >> 1]);
+            vstore<CW>(c.state + self_off + c.joff, xn);
+        }
+        __syncthreads();
+    }
+}
+
+// det32[] |= words with bit set where some spin of the clone has k != 0 (clone not in a ground
+// state).  Caller zeroes det32 and puts barriers around.
+template <int CW>
+__device__ __forceinline__ void tile_detect_acc(const TileCtx<CW>& c)
+{
+    uint32_t acc[2 * CW];
+#pragma unroll
+    for (int h = 0; h < 2 * CW; ++h) acc[h] = 0;
+    for (uint32_t p = c.slot; p < c.N; p += c.n_slots) {
+        uint32_t a[3][2 * CW], b[3][2 * CW], x[2 * CW], jm[3], self_off;
+        tile_gather<CW>(c, p, a, b, x, jm, self_off);
+#pragma unroll
+        for (int h = 0; h < 2 * CW; ++h)
+            acc[h] |= qg_nonzero_k(a[0][h], b[0][h], jm[0], a[1][h], b[1][h], jm[1], a[2][h], b[2][h],
+                                   jm[2], x[h]);
+    }
+#pragma unroll
+    for (int h = 0; h < 2 * CW; ++h)
+        if (acc[h]) atomicOr(&c.det32[2 * c.jw + h], acc[h]);
+}
+
+// Noise bytes for sweeps t_first .. t_first + ns - 1 (a-6).
+template <int CW>
+__device__ __forceinline__ void tile_produce(const TileCtx<CW>& c, uint32_t t_first, uint32_t ns,
+                                             uint32_t w0, uint32_t k0, uint32_t k1, uint32_t thr)
+{
+    const uint32_t G = c.T >= 4 ? c.T / 4 : 1;
+    const uint32_t per_sweep = c.N * G;
+    const uint32_t total = ns * per_sweep;
+    for (uint32_t e = threadIdx.x; e < total; e += blockDim.x) {
+        const uint32_t s = e / per_sweep;
+        const uint32_t q = e - s * per_sweep;
+        const uint32_t p = q / G, g = q - p * G;
+        const uint32_t spin = c.rec[3 * p + 1].w;
+        uint32_t o[4];
+        philox4x32_10(spin, (w0 >> 2) + g, t_first + s, TAG_SWEEP, k0, k1, o);
+        unsigned char* dst = c.rbuf + ((size_t)s * c.N + p) * c.T;
+        if (c.T >= 4) {
+            const uint32_t v = (o[0] < thr ? 0xFFu : 0u) | (o[1] < thr ? 0xFF00u : 0u) |
+                               (o[2] < thr ? 0xFF0000u : 0u) | (o[3] < thr ? 0xFF000000u : 0u);
+            *reinterpret_cast<uint32_t*>(dst + 4 * g) = v;
+        } else {
+            for (uint32_t lw = 0; lw < c.T; ++lw)
+                dst[lw] = o[(w0 + lw) & 3u] < thr ? 0xFF : 0;
+        }
+    }
+}
+
+template <int CW>
+__global__ void __launch_bounds__(1024, 1) k_sweep_tile(TileArgs A)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    const uint32_t N = A.N, W = A.W, T = A.T;
+    const uint32_t tiles = W / T;
+    const uint32_t inst = blockIdx.x / tiles;
+    const uint32_t w0 = (blockIdx.x % tiles) * T;
+    const xs_tts_rec rec0 = A.d.rec[inst];
+    if (rec0.solved && !(A.flags & XS_FLAG_NO_SKIP)) return;   // stop rule (L129, L293)
+
+    TileCtx<CW> c;
+    c.state = smem;
+    uint4* rec_w = reinterpret_cast<uint4*>(smem + A.off_rec);
+    c.rec = rec_w;
+    c.rbuf = smem + A.off_rbuf;
+    uint32_t* sets_w = reinterpret_cast<uint32_t*>(smem + A.off_sets);
+    c.sets = sets_w;
+    c.det32 = reinterpret_cast<uint32_t*>(smem + A.off_misc);
+    c.known32 = c.det32 + 2 * T;
+    c.flag = c.known32 + 2 * T;
+    c.N = N; c.T = T;
+    c.n_sets = A.d.n_sets[inst];
+    const uint32_t LPS = T / CW;
+    c.slot = threadIdx.x / LPS;
+    c.n_slots = blockDim.x / LPS;
+    c.jw = (threadIdx.x % LPS) * CW;
+    c.joff = c.jw * 8;
+
+    const uint64_t seed = A.d.run_seed[inst];
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    uint64_t* xg = A.d.x + (size_t)inst * N * W + w0;
+    uint32_t* fhg = A.d.first_hit + ((size_t)inst * W + w0) * 64;
+    const uint32_t row_bytes = T * 8;
+
+    // ---- a-3: tile load -------------------------------------------------------------------
+    const AdjRec* adj = A.d.adj + (size_t)inst * N;
+    for (uint32_t p = threadIdx.x; p < N; p += blockDim.x) {
+        const AdjRec r = adj[p];
+        rec_w[3 * p] = make_uint4(r.nbr[0] * row_bytes, r.nbr[1] * row_bytes, r.nbr[2] * row_bytes,
+                                  r.nbr[3] * row_bytes);
+        rec_w[3 * p + 1] = make_uint4(r.nbr[4] * row_bytes, r.nbr[5] * row_bytes, r.self * row_bytes,
+                                      r.self);
+        rec_w[3 * p + 2] = make_uint4((r.jbits & 1u) ? ~0u : 0u, (r.jbits & 2u) ? ~0u : 0u,
+                                      (r.jbits & 4u) ? ~0u : 0u, 0u);
+    }
+    for (uint32_t s = threadIdx.x; s <= c.n_sets; s += blockDim.x)
+        sets_w[s] = A.d.set_start[(size_t)inst * (N + 1) + s];
+    auto load_state = [&]() {
+        for (uint32_t e = threadIdx.x; e < N * T; e += blockDim.x) {
+            const uint32_t i = e / T, lw = e - i * T;
+            reinterpret_cast<uint64_t*>(smem)[e] = xg[(size_t)i * W + lw];
+        }
+    };
+    auto store_state = [&]() {
+        for (uint32_t e = threadIdx.x; e < N * T; e += blockDim.x) {
+            const uint32_t i = e / T, lw = e - i * T;
+            xg[(size_t)i * W + lw] = reinterpret_cast<const uint64_t*>(smem)[e];
+        }
+    };
+    load_state();
+    // known32: bit set <=> the clone already has a first-hit entry
+    for (uint32_t e = threadIdx.x; e < ((64 * T + 31) / 32) * 32; e += blockDim.x) {
+        const bool k = fhg[e] != XS_NO_HIT;
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, k);
+        if ((threadIdx.x & 31) == 0) c.known32[e >> 5] = m;
+    }
+    __syncthreads();
+
+    // solved mask of the current tile -> det32 (bit set = NOT solved); ends with a barrier
+    auto detect = [&]() {
+        for (uint32_t e = threadIdx.x; e < 2 * T; e += blockDim.x) c.det32[e] = 0;
+        if (threadIdx.x == 0) *c.flag = 0;
+        __syncthreads();
+        tile_detect_acc<CW>(c);
+        __syncthreads();
+    };
+    // sweeps t0+1 .. t0+n; exact: record first hits after every sweep
+    auto run_range = [&](uint32_t t0, uint32_t n, bool exact) {
+        for (uint32_t s0 = 0; s0 < n; s0 += A.rb) {
+            const uint32_t ns = min(A.rb, n - s0);
+            tile_produce<CW>(c, t0 + s0 + 1, ns, w0, k0, k1, A.thr);
+            __syncthreads();
+            for (uint32_t s = 0; s < ns; ++s) {
+                tile_sweep<CW>(c, s);
+                if (exact) {
+                    detect();
+                    const uint32_t t = t0 + s0 + s + 1;
+                    for (uint32_t e = threadIdx.x; e < 2 * T; e += blockDim.x) {
+                        uint32_t newly = ~c.det32[e] & ~c.known32[e];
+                        c.known32[e] |= newly;
+                        while (newly) {
+                            const int bit = __ffs(newly) - 1;
+                            newly &= newly - 1;
+                            fhg[32 * e + bit] = t;
+                        }
+                    }
+                    __syncthreads();
+                }
+            }
+        }
+    };
+
+    uint32_t t = (uint32_t)rec0.sweeps_done;
+    uint32_t remaining = A.n_sweeps;
+    while (remaining) {
+        const uint32_t nb = min(A.batch, remaining);
+        run_range(t, nb, false);
+        detect();
+        for (uint32_t e = threadIdx.x; e < 2 * T; e += blockDim.x)
+            if (~c.det32[e] & ~c.known32[e]) *c.flag = 1;
+        __syncthreads();
+        const bool replay = *c.flag != 0;
+        __syncthreads();
+        if (replay) {
+            load_state();          // global copy = state at the start of this batch
+            __syncthreads();
+            run_range(t, nb, true);
+        }
+        store_state();             // a-10 (also the replay checkpoint of the next batch)
+        t += nb;
+        remaining -= nb;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a-4 .. a-9: streaming regime (tile does not fit on chip, e.g. N = 2^20).
+// One launch per independent set; a lane owns CW words of one spin row and gathers the six
+// partner rows from global memory (HBM / L2).  Spins of a set are mutually non-adjacent
+// (L277), so the in-place update is race free inside a launch; launch order gives the set
+// order.  k != 0 words are OR-reduced per sweep into det[inst][w] (registers -> shared ->
+// one global atomic per CTA and word), and k_stream_commit turns clear bits into first hits.
+// ------------------------------------------------------------------------------------------
+constexpr uint32_t ST_THREADS = 256;
+
+template <int CW>
+__global__ void __launch_bounds__(ST_THREADS) k_stream_set(DevPtrs d, uint32_t N, uint32_t W,
+                                                          uint32_t set_idx, uint32_t s_rel,
+                                                          uint32_t thr, uint32_t flags, uint64_t* det)
+{
+    __shared__ uint32_t sdet[1024];
+    const uint32_t inst = blockIdx.y;
+    const xs_tts_rec rec = d.rec[inst];
+    if (rec.solved && !(flags & XS_FLAG_NO_SKIP)) return;
+    if (set_idx >= d.n_sets[inst]) return;
+    const uint32_t* ss = d.set_start + (size_t)inst * (N + 1);
+    const uint32_t p0 = ss[set_idx], p1 = ss[set_idx + 1];
+    const uint32_t nchunk = W / CW;
+    const uint64_t total = (uint64_t)(p1 - p0) * nchunk;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const bool fixed = (stride % nchunk == 0) && (2 * W <= 1024);
+    const uint32_t t = (uint32_t)rec.sweeps_done + s_rel;
+    const uint64_t seed = d.run_seed[inst];
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    uint64_t* x = d.x + (size_t)inst * N * W;
+    uint32_t* det32 = reinterpret_cast<uint32_t*>(det + (size_t)inst * W);
+    const AdjRec* adj = d.adj + (size_t)inst * N;
+
+    if (fixed) {
+        for (uint32_t e = threadIdx.x; e < 2 * W; e += blockDim.x) sdet[e] = 0;
+        __syncthreads();
+    }
+    uint32_t acc[2 * CW];
+#pragma unroll
+    for (int h = 0; h < 2 * CW; ++h) acc[h] = 0;
+    uint32_t my_w = 0;
+    for (uint64_t task = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; task < total; task += stride) {
+        const uint32_t q = (uint32_t)(task / nchunk);
+        const uint32_t ch = (uint32_t)(task - (uint64_t)q * nchunk);
+        const uint32_t w = ch * CW;
+        my_w = w;
+        const uint4* rp = reinterpret_cast<const uint4*>(adj + p0 + q);
+        const uint4 r0 = __ldg(rp), r1 = __ldg(rp + 1);
+        uint32_t a[3][2 * CW], b[3][2 * CW], xo[2 * CW];
+        vload<CW>(x + (size_t)r0.x * W + w, a[0]);
+        vload<CW>(x + (size_t)r0.y * W + w, b[0]);
+        vload<CW>(x + (size_t)r0.z * W + w, a[1]);
+        vload<CW>(x + (size_t)r0.w * W + w, b[1]);
+        vload<CW>(x + (size_t)r1.x * W + w, a[2]);
+        vload<CW>(x + (size_t)r1.y * W + w, b[2]);
+        uint64_t* own = x + (size_t)r1.z * W + w;
+        vload<CW>(own, xo);
+        const uint32_t jm0 = (r1.w & 1u) ? ~0u : 0u, jm1 = (r1.w & 2u) ? ~0u : 0u,
+                       jm2 = (r1.w & 4u) ? ~0u : 0u;
+        uint32_t o[4];
+        philox4x32_10(r1.z, w >> 2, t, TAG_SWEEP, k0, k1, o);
+        uint32_t xn[2 * CW];
+#pragma unroll
+        for (int h = 0; h < 2 * CW; ++h) {
+            const uint32_t R = o[(w + (h >> 1)) & 3u] < thr ? ~0u : 0u;
+            const uint32_t nz = qg_nonzero_k(a[0][h], b[0][h], jm0, a[1][h], b[1][h], jm1, a[2][h],
+                                             b[2][h], jm2, xo[h]);
+            xn[h] = qg_update(a[0][h], b[0][h], jm0, a[1][h], b[1][h], jm1, a[2][h], b[2][h], jm2,
+                              xo[h], R);
+            if (fixed) acc[h] |= nz;
+            else if (nz) atomicOr(&det32[2 * w + h], nz);
+        }
+        vstore<CW>(own, xn);
+    }
+    if (fixed) {
+#pragma unroll
+        for (int h = 0; h < 2 * CW; ++h)
+            if (acc[h]) atomicOr(&sdet[2 * my_w + h], acc[h]);
+        __syncthreads();
+        for (uint32_t e = threadIdx.x; e < 2 * W; e += blockDim.x)
+            if (sdet[e]) atomicOr(&det32[e], sdet[e]);
+    }
+}
+
+// After the last set of relative sweep s_rel: a clear bit in det_cur means every spin of the
+// clone saw k = 0 during the sweep, i.e. the clone was in a ground state when the sweep
+// started -> first hit = t - 1.  Also clears det_next for the following sweep.
+__global__ void k_stream_commit(DevPtrs d, uint32_t W, uint32_t I, const uint64_t* det_cur,
+                                uint64_t* det_next, uint32_t s_rel, uint32_t flags)
+{
+    const uint64_t total = (uint64_t)I * W * 64;
+    for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t inst = (uint32_t)(e / ((uint64_t)W * 64));
+        const xs_tts_rec rec = d.rec[inst];
+        if (!(rec.solved && !(flags & XS_FLAG_NO_SKIP))) {
+            const bool solved = ((det_cur[e >> 6] >> (e & 63)) & 1ull) == 0;
+            if (solved && d.first_hit[e] == XS_NO_HIT)
+                d.first_hit[e] = (uint32_t)rec.sweeps_done + s_rel - 1u;
+        }
+        if (e < (uint64_t)I * W) det_next[e] = 0;
+    }
+}
+
+// first-hit marking at the end of a streaming call for instances that were swept
+__global__ void k_mark_swept(DevPtrs d, uint32_t W, uint32_t I, const uint64_t* det,
+                             uint32_t n_sweeps, uint32_t flags)
+{
+    const uint64_t total = (uint64_t)I * W * 64;
+    for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t inst = (uint32_t)(e / ((uint64_t)W * 64));
+        const xs_tts_rec rec = d.rec[inst];
+        if (rec.solved && !(flags & XS_FLAG_NO_SKIP)) continue;
+        const bool solved = ((det[e >> 6] >> (e & 63)) & 1ull) == 0;
+        if (solved && d.first_hit[e] == XS_NO_HIT)
+            d.first_hit[e] = (uint32_t)rec.sweeps_done + n_sweeps;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// host side: geometry and launchers
+// ------------------------------------------------------------------------------------------
+namespace {
+constexpr uint32_t SMEM_MAX = 227u * 1024u;   // per-CTA opt-in limit on sm_100a
+constexpr uint32_t NUM_SMS = 148;
+
+inline uint32_t round_up(uint32_t v, uint32_t m) { return (v + m - 1) / m * m; }
+inline uint32_t env_u32(const char* name, uint32_t dflt)
+{
+    const char* s = std::getenv(name);
+    return (s && *s) ? (uint32_t)std::strtoul(s, nullptr, 10) : dflt;
+}
+
+struct TileSmem { uint32_t off_rec, off_rbuf, off_sets, off_misc, total; };
+TileSmem tile_smem(uint32_t N, uint32_t T, uint32_t rb, uint32_t n_sets_max)
+{
+    TileSmem s;
+    uint64_t o = (uint64_t)N * T * 8;
+    s.off_rec = (uint32_t)o;           o += (uint64_t)N * 48;
+    s.off_rbuf = (uint32_t)o;          o += round_up(rb * N * T, 16);
+    s.off_sets = (uint32_t)o;          o += round_up((n_sets_max + 1) * 4, 16);
+    s.off_misc = (uint32_t)o;          o += round_up((4 * T + 4) * 4, 16);
+    s.total = o > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)o;
+    return s;
+}
+}  // namespace
+
+bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
+{
+    const xs_params& p = b.p;
+    g = TileGeom{};
+    g.batch = std::max(1u, env_u32("XS_BATCH", 64));
+    const uint32_t force_T = env_u32("XS_TILE_WORDS", 0);
+    uint32_t bestT = 0;
+    uint64_t best_cost = ~0ull;
+    if (!(p.flags & XS_FLAG_STREAMING) && (uint64_t)p.n_spins * 8 < SMEM_MAX) {
+        for (uint32_t T = 64; T >= 1; T >>= 1) {
+            if (p.n_words % T) continue;
+            if (force_T && T != force_T) continue;
+            const TileSmem s = tile_smem(p.n_spins, T, 1, b.n_sets_max);
+            if (s.total > SMEM_MAX) continue;
+            const uint64_t ctas = (uint64_t)p.n_instances * (p.n_words / T);
+            const uint32_t occ = std::max(1u, std::min(SMEM_MAX / s.total, 2048u / 1024u));
+            const uint64_t waves = (ctas + (uint64_t)NUM_SMS * occ - 1) / ((uint64_t)NUM_SMS * occ);
+            const uint64_t cost = waves * T * occ;
+            if (cost < best_cost) { best_cost = cost; bestT = T; }
+        }
+    }
+    if (bestT == 0) {
+        g.regime = 1;
+        g.T = p.n_words;
+        g.CW = (p.n_words % 2 == 0) ? 2 : 1;
+        g.threads = ST_THREADS;
+        const uint64_t tasks = (uint64_t)b.max_set_size * (p.n_words / g.CW);
+        g.ctas = (uint32_t)std::min<uint64_t>((tasks + ST_THREADS - 1) / ST_THREADS, NUM_SMS * 8);
+        g.ctas = std::max(g.ctas, 1u);
+        g.smem = 0;
+        g.batch = 1;
+        g.rb = 0;
+        (void)err;
+        return true;
+    }
+    g.regime = 0;
+    g.T = bestT;
+    g.CW = bestT >= 2 ? 2 : 1;
+    const uint32_t LPS = g.T / g.CW;
+    const uint32_t want = round_up(std::max(b.max_set_size, 1u) * LPS, 32);
+    g.threads = std::min(1024u, std::max(128u, want));
+    g.threads = std::min(1024u, std::max(32u, env_u32("XS_THREADS", g.threads) / 32 * 32));
+    g.ctas = p.n_instances * (p.n_words / g.T);
+    uint32_t rb = std::min(g.batch, env_u32("XS_RB", 8));
+    while (rb > 1 && tile_smem(p.n_spins, g.T, rb, b.n_sets_max).total > SMEM_MAX) --rb;
+    g.rb = rb;
+    g.smem = tile_smem(p.n_spins, g.T, rb, b.n_sets_max).total;
+    return true;
+}
+
+#define XS_CU(call)                                         \
+    do {                                                    \
+        cudaError_t e_ = (call);                            \
+        if (e_ != cudaSuccess) return (int)e_;              \
+    } while (0)
+
+static inline uint32_t grid_for(uint64_t total, uint32_t threads)
+{
+    return (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>((total + threads - 1) / threads, NUM_SMS * 16));
+}
+
+int launch_init(const xs_batch& b, void* stream)
+{
+    const xs_params& p = b.p;
+    const uint64_t total = (uint64_t)p.n_instances * p.n_spins * p.n_words;
+    k_init<<<grid_for(total, 256), 256, 0, (cudaStream_t)stream>>>(b.d, p.n_spins, p.n_words, p.n_instances);
+    return (int)cudaGetLastError();
+}
+
+// det slot 0 <- unsat OR of the current global state
+static int launch_unsat_or(const xs_batch& b, cudaStream_t st)
+{
+    const xs_params& p = b.p;
+    XS_CU(cudaMemsetAsync(b.d.det, 0, (size_t)p.n_instances * p.n_words * 8, st));
+    dim3 grid((p.n_spins + DET_CHUNK - 1) / DET_CHUNK, p.n_instances);
+    const uint32_t thr = std::min(256u, round_up(p.n_words, 32));
+    k_unsat_or<<<grid, thr, 0, st>>>(b.d, p.n_spins, p.n_words, b.d.det);
+    return (int)cudaGetLastError();
+}
+
+int launch_mark(const xs_batch& b, bool reset_first_hit, void* stream)
+{
+    const xs_params& p = b.p;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = launch_unsat_or(b, st);
+    if (rc) return rc;
+    const uint64_t total = (uint64_t)p.n_instances * p.n_words * 64;
+    k_mark<<<grid_for(total, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, b.d.det,
+                                                 reset_first_hit ? 1 : 0, 0u);
+    return (int)cudaGetLastError();
+}
+
+int launch_finalize(const xs_batch& b, uint32_t n_sweeps, void* stream)
+{
+    k_finalize<<<b.p.n_instances, 256, 0, (cudaStream_t)stream>>>(b.d, b.p.n_words, n_sweeps, b.p.flags);
+    return (int)cudaGetLastError();
+}
+
+int launch_energy(const xs_batch& b, int32_t* dev_out, void* stream)
+{
+    const xs_params& p = b.p;
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint64_t total = (uint64_t)p.n_instances * p.n_words * 64;
+    k_energy_fill<<<grid_for(total, 256), 256, 0, st>>>(dev_out, total, -(int32_t)p.n_spins);
+    dim3 grid(p.n_words, p.n_instances, (p.n_spins + EN_CHUNK - 1) / EN_CHUNK);
+    k_energy_acc<<<grid, EN_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, dev_out);
+    return (int)cudaGetLastError();
+}
+
+int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
+{
+    const xs_params& p = b.p;
+    const TileGeom& g = b.geom;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n_sweeps == 0) return 0;
+    if (g.regime == 0) {
+        const TileSmem s = tile_smem(p.n_spins, g.T, g.rb, b.n_sets_max);
+        TileArgs A;
+        A.d = b.d;
+        A.N = p.n_spins; A.W = p.n_words; A.T = g.T; A.n_sweeps = n_sweeps;
+        A.thr = p.w1_threshold; A.flags = p.flags; A.batch = g.batch; A.rb = g.rb;
+        A.off_rec = s.off_rec; A.off_rbuf = s.off_rbuf; A.off_sets = s.off_sets; A.off_misc = s.off_misc;
+        if (g.CW == 2) {
+            XS_CU(cudaFuncSetAttribute(k_sweep_tile<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.total));
+            k_sweep_tile<2><<<g.ctas, g.threads, s.total, st>>>(A);
+        } else {
+            XS_CU(cudaFuncSetAttribute(k_sweep_tile<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.total));
+            k_sweep_tile<1><<<g.ctas, g.threads, s.total, st>>>(A);
+        }
+        return (int)cudaGetLastError();
+    }
+    // streaming regime
+    const size_t det_words = (size_t)p.n_instances * p.n_words;
+    uint64_t* det[2] = {b.d.det, b.d.det + det_words};
+    XS_CU(cudaMemsetAsync(b.d.det, 0, 2 * det_words * 8, st));
+    dim3 grid(g.ctas, p.n_instances);
+    const uint64_t clones = det_words * 64;
+    for (uint32_t s = 1; s <= n_sweeps; ++s) {
+        uint64_t* cur = det[s & 1];
+        for (uint32_t set = 0; set < b.n_sets_max; ++set) {
+            if (g.CW == 2)
+                k_stream_set<2><<<grid, ST_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, set, s,
+                                                             p.w1_threshold, p.flags, cur);
+            else
+                k_stream_set<1><<<grid, ST_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, set, s,
+                                                             p.w1_threshold, p.flags, cur);
+        }
+        k_stream_commit<<<grid_for(clones, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, cur,
+                                                              det[(s + 1) & 1], s, p.flags);
+        XS_CU(cudaGetLastError());
+    }
+    int rc = launch_unsat_or(b, st);
+    if (rc) return rc;
+    k_mark_swept<<<grid_for(clones, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, b.d.det,
+                                                       n_sweeps, p.flags);
+    return (int)cudaGetLastError();
+}
+
+}  // namespace xs

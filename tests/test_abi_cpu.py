@@ -1,0 +1,102 @@
+"""CPU-side checks of the product library: it loads, exports every symbol include/xs.h declares,
+its host generator agrees byte for byte with the (independently written) oracle generator, its
+TTS statistics match closed forms / scipy, and argument errors come back as codes.
+No kernel is launched here."""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2102_09510_b200 as xs
+from oracle.xs_oracle import Instance
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "xs.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(xs_[a-z_0-9]+)\s*\(", hdr))
+    assert {"xs_create_instance", "xs_run_sweeps", "xs_energy", "xs_tts"} <= declared
+    L = xs.lib()
+    for name in sorted(declared):
+        assert hasattr(L, name), f"libxs_b200.so does not export {name}"
+    from paper_2102_09510_b200 import _binding
+    assert declared == set(_binding.EXPORTS)
+
+
+@pytest.mark.parametrize("N,seed,cap,gauge", [(64, 1, 0, True), (256, 2, 0, True), (512, 100, 0, True),
+                                              (512, 101, 32, True), (20, 7, 0, False), (999, 5, 3, True),
+                                              (3, 1, 0, True), (4096, 9, 0, True)])
+def test_generator_matches_oracle_generator(N, seed, cap, gauge):
+    tri, jbit, order, ss, att = xs.xs_generate_graph(N, seed, xs.XS_FLAG_GAUGE if gauge else 0, cap)
+    o = Instance(N, seed, gauge, cap)
+    assert att == o.attempt
+    assert np.array_equal(tri, o.tri)
+    assert np.array_equal(jbit, o.jbit)
+    assert np.array_equal(order, o.order)
+    assert np.array_equal(ss, o.set_size)
+    assert o.check_order(order, ss)
+
+
+def test_workspace_bytes_and_param_errors():
+    p = xs.make_params(256, 1024, 1)
+    n = xs.xs_workspace_bytes(p)
+    assert n >= 256 * 1024 * 8 + 65536 * 4
+    for bad in [xs.make_params(2, 1, 1), xs.make_params(64, 0, 1), xs.make_params(64, 1, 0)]:
+        with pytest.raises(xs.XsError) as ei:
+            xs.xs_workspace_bytes(bad)
+        assert ei.value.code == -1
+    L = xs.lib()
+    assert L.xs_run_sweeps(None, 1, None) == -1
+    assert b"null" in L.xs_last_error()
+    assert L.xs_destroy(None) == 0
+
+
+def test_tts_stats_closed_forms():
+    """L113 Eq.(2), L117/L123: TTS_p = -ln(1-p/100) tau; L145 posterior = inverse-gamma(n, T_tot)."""
+    scipy_stats = pytest.importorskip("scipy.stats")
+    rng = np.random.default_rng(0)
+    tts = rng.exponential(5000.0, 400).astype(np.uint32) + 1
+    s = xs.xs_tts_stats(tts, 0)
+    assert s["n_solved"] == 400 and s["t_tot"] == float(tts.sum())
+    assert s["tau_hat"] == pytest.approx(tts.mean(), rel=1e-12)
+    for p, key in [(0.5, "tts50_model"), (0.9, "tts90_model"), (0.99, "tts99_model")]:
+        assert s[key] == pytest.approx(-math.log(1 - p) * tts.mean(), rel=1e-12)
+    srt = np.sort(tts)
+    assert s["tts50_emp"] == srt[199] and s["tts90_emp"] == srt[359] and s["tts99_emp"] == srt[395]
+    # with a timeout: censored runs count t_max each
+    t_max = 3000
+    cens = np.where(tts <= t_max, tts, xs.XS_NO_HIT).astype(np.uint32)
+    c = xs.xs_tts_stats(cens, t_max)
+    n = int((tts <= t_max).sum())
+    t_tot = float(tts[tts <= t_max].sum() + (400 - n) * t_max)
+    assert c["n_solved"] == n and c["t_tot"] == t_tot
+    assert c["tau_hat"] == pytest.approx(t_tot / n)
+    ig = scipy_stats.invgamma(a=n, scale=t_tot)
+    assert c["tau_q16"] == pytest.approx(ig.ppf(0.16), rel=1e-6)
+    assert c["tau_q50"] == pytest.approx(ig.ppf(0.50), rel=1e-6)
+    assert c["tau_q84"] == pytest.approx(ig.ppf(0.84), rel=1e-6)
+    assert math.isinf(c["tts99_emp"])
+    # the censored estimate recovers the true scale within its own error bar
+    assert c["tau_q16"] < 5000.0 * 1.15 and c["tau_q84"] > 5000.0 * 0.85
+    # nothing solved: only a lower bound
+    z = xs.xs_tts_stats(np.full(10, xs.XS_NO_HIT, np.uint32), 1000)
+    assert z["n_solved"] == 0 and math.isinf(z["tau_hat"])
+    assert z["tau_q16"] == pytest.approx(10 * 1000 / math.log(20.0))
+    # n = 1: inverse-gamma(1, T): median = T / ln 2
+    one = xs.xs_tts_stats(np.array([700], np.uint32), 0)
+    assert one["tau_q50"] == pytest.approx(700 / math.log(2.0), rel=1e-9)
+
+
+def test_no_cpu_fallback_without_gpu():
+    torch = pytest.importorskip("torch")
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(RuntimeError):
+        xs.Batch(64, 1, [1], [1])

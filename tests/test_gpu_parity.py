@@ -1,0 +1,241 @@
+"""GPU-vs-oracle parity through the C ABI (bit-exact: spin words, energies, first-hit sweeps).
+
+Protocol: SURVEY.md 8(c) "GPU-vs-oracle parity protocol" -- words evolve independently given
+(seed, w) because the noise is counter based, so (i) all words for a moderate number of sweeps,
+(ii) sampled words for the long runs at full size.  Tolerance: none; this is integer work.
+"""
+from __future__ import annotations
+
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from _harness import OracleRun  # noqa: E402
+from oracle.xs_oracle import NO_HIT, Instance  # noqa: E402
+
+
+def _xs():
+    import paper_2102_09510_b200 as xs
+    return xs
+
+
+@pytest.fixture(autouse=True)
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
+
+
+class env:
+    """Temporarily set geometry knobs the library reads at xs_create_instance time."""
+
+    def __init__(self, **kw):
+        self.kw = {k: str(v) for k, v in kw.items()}
+
+    def __enter__(self):
+        self.old = {k: os.environ.get(k) for k in self.kw}
+        os.environ.update(self.kw)
+
+    def __exit__(self, *a):
+        for k, v in self.old.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+
+
+def _compare(b, oracles, what=""):
+    """b: xs.Batch; oracles: list of OracleRun, one per instance."""
+    x = b.spins_numpy()
+    fh = b.first_hit_numpy()
+    e = b.energy().cpu().numpy()
+    recs = b.tts()
+    for i, o in enumerate(oracles):
+        xo = o.x()
+        eo = o.energy()
+        for w in o.words:
+            assert np.array_equal(x[i, :, w], xo[:, w]), f"{what}: spins differ inst {i} word {w}"
+            sl = slice(64 * w, 64 * w + 64)
+            assert np.array_equal(fh[i, sl], o.first_hit[sl]), f"{what}: first_hit differ inst {i} word {w}"
+            assert np.array_equal(e[i, sl], eo[sl]), f"{what}: energies differ inst {i} word {w}"
+        if len(o.words) == o.W:
+            solved, tts, clone = o.tts()
+            assert (recs[i].solved, recs[i].tts_sweeps, recs[i].clone) == (solved, tts, clone), what
+        assert recs[i].sweeps_done == o.sweeps_done, f"{what}: sweeps_done inst {i}"
+
+
+def test_init_state_and_energy():
+    xs = _xs()
+    for N, W, gs, rs in [(64, 3, 1, 1), (200, 8, 11, 12)]:
+        b = xs.Batch(N, W, [gs], [rs])
+        o = OracleRun(N, W, gs, rs)
+        _compare(b, [o], f"init N={N}")
+        b.close()
+
+
+@pytest.mark.parametrize("N,W,sweeps,tile", [
+    (64, 1, 300, 0),      # config-1 shape: one word, CW=1 path
+    (96, 4, 120, 0),
+    (96, 6, 60, 0),       # W not a power of two -> T = 2
+    (256, 8, 40, 8),      # config-2 tile shape (T = 8)
+    (256, 16, 24, 16),
+    (130, 32, 20, 32),
+    (70, 64, 12, 64),
+    (512, 32, 8, 32),     # config-3 tile shape
+])
+def test_sweep_parity_all_words(N, W, sweeps, tile):
+    xs = _xs()
+    with env(XS_TILE_WORDS=tile, XS_BATCH=16):
+        b = xs.Batch(N, W, [N + 7], [3 * N + 1], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
+    if tile:
+        assert b.layout().tile_words == tile and b.layout().regime == 0
+    o = OracleRun(N, W, N + 7, 3 * N + 1, no_skip=True)
+    half = sweeps // 3
+    for n in (half, sweeps - half):          # two calls: resume must be exact
+        b.run_sweeps(n)
+        o.run_sweeps(n)
+    _compare(b, [o], f"N={N} W={W}")
+    b.close()
+
+
+def test_config1_until_solved_matches_oracle_and_survey_hint(golden):
+    """BASELINE.json configs[0]: N=64, seed 1, 64 clones, until E=-N, K=100 sweeps per call."""
+    xs = _xs()
+    hint = dict(line.split(None, 1) for line in open(golden("config1_survey_hint.txt"))
+                if line.strip() and not line.startswith("#"))
+    b = xs.Batch(64, 1, [1], [1])
+    o = OracleRun(64, 1, 1, 1)
+    for _ in range(1000):
+        b.run_sweeps(100)
+        o.run_sweeps(100)
+        if b.tts()[0].solved:
+            break
+    _compare(b, [o], "config 1")
+    r = b.tts()[0]
+    assert r.solved == 1
+    assert r.tts_sweeps == int(hint["first_hit_sweep"]) and r.clone == int(hint["first_hit_clone"])
+    # skipped once solved: further calls change nothing
+    x0 = b.spins_numpy().copy()
+    b.run_sweeps(100)
+    o.run_sweeps(100)
+    assert np.array_equal(b.spins_numpy(), x0)
+    _compare(b, [o], "config 1 after solve")
+    b.close()
+
+
+@pytest.mark.parametrize("batch", [1, 5, 64])
+@pytest.mark.parametrize("streaming", [False, True])
+def test_first_hit_exact_many_solved_clones(batch, streaming):
+    """Small N: clones solve all the time -> exercises the in-kernel replay at every batch."""
+    xs = _xs()
+    N, W = 18, 4
+    flags = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_STREAMING if streaming else 0)
+    with env(XS_BATCH=batch):
+        b = xs.Batch(N, W, [5], [9], flags=flags)
+    assert b.layout().regime == (1 if streaming else 0)
+    o = OracleRun(N, W, 5, 9, no_skip=True)
+    for n in (1, 7, 30, 13):
+        b.run_sweeps(n)
+        o.run_sweeps(n)
+        _compare(b, [o], f"batch={batch} streaming={streaming}")
+    assert (o.first_hit != NO_HIT).sum() > 20
+    b.close()
+
+
+def test_streaming_regime_matches_oracle():
+    xs = _xs()
+    for N, W, sweeps in [(96, 16, 12), (150, 3, 10), (64, 2, 30)]:
+        b = xs.Batch(N, W, [N], [N + 1], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_STREAMING)
+        assert b.layout().regime == 1
+        o = OracleRun(N, W, N, N + 1, no_skip=True)
+        b.run_sweeps(sweeps)
+        o.run_sweeps(sweeps)
+        _compare(b, [o], f"streaming N={N} W={W}")
+        b.close()
+
+
+def test_multi_instance_stop_rule():
+    """Instances that have a solved clone at call entry are skipped (L129/L293 stop rule)."""
+    xs = _xs()
+    N, W = 32, 1
+    gseeds = list(range(3, 11))
+    rseeds = list(range(13, 21))
+    b = xs.Batch(N, W, gseeds, rseeds)
+    os_ = [OracleRun(N, W, g, r) for g, r in zip(gseeds, rseeds)]
+    for _ in range(10):
+        b.run_sweeps(20)
+        for o in os_:
+            o.run_sweeps(20)
+        _compare(b, os_, "stop rule")
+    done = [o.sweeps_done for o in os_]
+    assert len(set(done)) > 1, "test should see instances stopping at different times"
+    b.close()
+
+
+def test_from_arrays_cap32_and_frustrated_couplings():
+    """Paper-faithful cap-32 sets (L279) and arbitrary J (no planted solution)."""
+    xs = _xs()
+    N, W = 160, 4
+    inst = Instance(N, 77, gauge=True, set_cap=32)
+    rng = np.random.default_rng(5)
+    jbit = rng.integers(0, 2, N).astype(np.uint8)
+    inst2 = Instance(N, 77, set_cap=32, tri=inst.tri, jbit=jbit)
+    arrays = (inst2.tri[None], jbit[None], inst2.order[None], inst2.set_size[None],
+              np.array([inst2.n_sets], np.uint32))
+    b = xs.Batch(N, W, run_seeds=[21], arrays=arrays, flags=xs.XS_FLAG_NO_SKIP)
+    o = OracleRun(N, W, 77, 21, no_skip=True, inst=inst2)
+    b.run_sweeps(25)
+    o.run_sweeps(25)
+    _compare(b, [o], "from arrays")
+    tri, jb, order, ss = b.get_graph(0)
+    assert np.array_equal(tri, inst2.tri) and np.array_equal(order, inst2.order)
+    assert np.array_equal(ss, inst2.set_size) and np.array_equal(jb, jbit)
+    b.close()
+
+
+def test_gauge_covariance_on_gpu():
+    """Run A (J=+1, x0) vs run B (planted J, x0 ^ taubit): x_B(t) = x_A(t) ^ taubit (L43)."""
+    xs = _xs()
+    N, W = 80, 4
+    a = xs.Batch(N, W, [31], [5], flags=xs.XS_FLAG_NO_SKIP)                       # ferromagnet
+    g = xs.Batch(N, W, [31], [5], flags=xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_GAUGE)    # gauged
+    taubit = Instance(N, 31, gauge=True).taubit.astype(np.uint64)
+    mask = (taubit * np.uint64(0xFFFFFFFFFFFFFFFF))[None, :, None]
+    x0 = a.spins_numpy()
+    g.set_spins(torch.from_numpy((x0 ^ mask).view(np.int64)).cuda())
+    a.run_sweeps(50)
+    g.run_sweeps(50)
+    assert np.array_equal(g.spins_numpy(), a.spins_numpy() ^ mask)
+    assert np.array_equal(g.energy().cpu().numpy(), a.energy().cpu().numpy())
+    assert np.array_equal(g.first_hit_numpy(), a.first_hit_numpy())
+    a.close()
+    g.close()
+
+
+def test_set_spins_planted_state_is_ground_state():
+    xs = _xs()
+    N, W = 100, 2
+    b = xs.Batch(N, W, [8], [8])
+    taubit = Instance(N, 8, gauge=True).taubit.astype(np.uint64)
+    x = np.zeros((1, N, W), np.uint64)
+    x[0, :, 0] = taubit * np.uint64(1 << 5)      # clone 5 = planted state, others all +1
+    b.set_spins(torch.from_numpy(x.view(np.int64)).cuda())
+    e = b.energy().cpu().numpy()[0]
+    assert e[5] == -N
+    r = b.tts()[0]
+    fh = b.first_hit_numpy()[0]
+    assert fh[5] == 0 and r.solved == 1 and r.tts_sweeps == 0 and r.clone <= 5
+    b.close()
+
+
+def test_error_codes_on_gpu():
+    xs = _xs()
+    p = xs.make_params(64, 1, 1)
+    ws = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(xs.XsError) as ei:
+        xs.xs_create_instance(p, [1], [1], ws.data_ptr() // 256 * 256 + 256, 16)
+    assert ei.value.code == -2
