@@ -162,6 +162,15 @@ int xs_get_layout(const xs_batch* b, xs_layout* out);
  *               scale T_tot) (L145); for n = 0, out[9] = T_tot / ln 20 (95 % lower bound), rest inf. */
 int xs_tts_stats(const uint32_t* tts, uint32_t n_runs, uint64_t t_max, double* out /* [12] */);
 
+/* Measurement helpers (no arithmetic of the method).
+ * xs_alu_peak: runs a pure-LOP3 micro-kernel (16 independent chains per thread, all SMs) and
+ *   returns the measured integer-pipe rate in 32-bit lane-operations per nanosecond for the
+ *   whole GPU -- the denominator of the integer-pipe roofline ("P_ALU is
+ *   measured").  Synchronises cuda_stream; allocates 4 bytes of device memory for its sink.
+ * xs_kernel_launches: kernels launched by this library in this process so far. */
+int xs_alu_peak(double* lane_ops_per_ns, double* kernel_ms, void* cuda_stream);
+uint64_t xs_kernel_launches(void);
+
 int xs_destroy(xs_batch* b);
 
 const char* xs_last_error(void);

@@ -8,7 +8,8 @@ from __future__ import annotations
 import numpy as np
 
 from ._binding import (XS_FLAG_GAUGE, XS_FLAG_NO_SKIP, XS_FLAG_STREAMING, XS_NO_HIT,  # noqa: F401
-                       XS_W1_THRESHOLD_DEFAULT, XsError, lib, make_params, xs_create_instance,
+                       XS_W1_THRESHOLD_DEFAULT, XsError, lib, make_params, xs_alu_peak,
+                       xs_create_instance, xs_kernel_launches,
                        xs_create_instance_from_arrays, xs_destroy, xs_energy, xs_get_first_hit,
                        xs_generate_graph, xs_get_graph, xs_get_layout, xs_get_spins, xs_params, xs_run_sweeps,
                        xs_set_spins, xs_tts, xs_tts_rec, xs_tts_stats, xs_workspace_bytes)

@@ -37,7 +37,8 @@ class xs_layout(C.Structure):
 
 EXPORTS = ["xs_workspace_bytes", "xs_create_instance", "xs_create_instance_from_arrays",
            "xs_run_sweeps", "xs_energy", "xs_tts", "xs_get_spins", "xs_set_spins",
-           "xs_get_first_hit", "xs_get_graph", "xs_generate_graph", "xs_get_layout", "xs_tts_stats", "xs_destroy",
+           "xs_get_first_hit", "xs_get_graph", "xs_generate_graph", "xs_get_layout", "xs_tts_stats",
+           "xs_alu_peak", "xs_kernel_launches", "xs_destroy",
            "xs_last_error"]
 
 _lib = None
@@ -70,10 +71,13 @@ def lib():
     L.xs_get_layout.argtypes = [vp, C.POINTER(xs_layout)]
     L.xs_tts_stats.argtypes = [u32p, C.c_uint32, C.c_uint64, C.POINTER(C.c_double)]
     L.xs_destroy.argtypes = [vp]
+    L.xs_alu_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
+    L.xs_kernel_launches.argtypes = []
     L.xs_last_error.restype = C.c_char_p
     for name in EXPORTS:
-        if name != "xs_last_error":
+        if name not in ("xs_last_error", "xs_kernel_launches"):
             getattr(L, name).restype = C.c_int
+    L.xs_kernel_launches.restype = C.c_uint64
     _lib = L
     return L
 
@@ -212,6 +216,17 @@ def xs_tts_stats(tts, t_max: int) -> dict:
     keys = ["n_solved", "t_tot", "tau_hat", "tts50_model", "tts90_model", "tts99_model",
             "tts50_emp", "tts90_emp", "tts99_emp", "tau_q16", "tau_q50", "tau_q84"]
     return dict(zip(keys, [float(v) for v in out]))
+
+
+def xs_alu_peak(stream=None):
+    """(lane-ops per ns of the whole GPU, kernel ms) from the LOP3 micro-kernel."""
+    v, ms = C.c_double(0), C.c_double(0)
+    _check(lib().xs_alu_peak(C.byref(v), C.byref(ms), _stream(stream)), "xs_alu_peak")
+    return float(v.value), float(ms.value)
+
+
+def xs_kernel_launches() -> int:
+    return int(lib().xs_kernel_launches())
 
 
 def xs_destroy(h):

@@ -730,6 +730,8 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
         if (e_ != cudaSuccess) return (int)e_;              \
     } while (0)
 
+void count_launch(uint64_t n);   // xs_diag.cu
+
 static inline uint32_t grid_for(uint64_t total, uint32_t threads)
 {
     return (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>((total + threads - 1) / threads, NUM_SMS * 16));
@@ -740,6 +742,7 @@ int launch_init(const xs_batch& b, void* stream)
     const xs_params& p = b.p;
     const uint64_t total = (uint64_t)p.n_instances * p.n_spins * p.n_words;
     k_init<<<grid_for(total, 256), 256, 0, (cudaStream_t)stream>>>(b.d, p.n_spins, p.n_words, p.n_instances);
+    count_launch(1);
     return (int)cudaGetLastError();
 }
 
@@ -751,6 +754,7 @@ static int launch_unsat_or(const xs_batch& b, cudaStream_t st)
     dim3 grid((p.n_spins + DET_CHUNK - 1) / DET_CHUNK, p.n_instances);
     const uint32_t thr = std::min(256u, round_up(p.n_words, 32));
     k_unsat_or<<<grid, thr, 0, st>>>(b.d, p.n_spins, p.n_words, b.d.det);
+    count_launch(1);
     return (int)cudaGetLastError();
 }
 
@@ -763,12 +767,14 @@ int launch_mark(const xs_batch& b, bool reset_first_hit, void* stream)
     const uint64_t total = (uint64_t)p.n_instances * p.n_words * 64;
     k_mark<<<grid_for(total, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, b.d.det,
                                                  reset_first_hit ? 1 : 0, 0u);
+    count_launch(1);
     return (int)cudaGetLastError();
 }
 
 int launch_finalize(const xs_batch& b, uint32_t n_sweeps, void* stream)
 {
     k_finalize<<<b.p.n_instances, 256, 0, (cudaStream_t)stream>>>(b.d, b.p.n_words, n_sweeps, b.p.flags);
+    count_launch(1);
     return (int)cudaGetLastError();
 }
 
@@ -778,8 +784,10 @@ int launch_energy(const xs_batch& b, int32_t* dev_out, void* stream)
     cudaStream_t st = (cudaStream_t)stream;
     const uint64_t total = (uint64_t)p.n_instances * p.n_words * 64;
     k_energy_fill<<<grid_for(total, 256), 256, 0, st>>>(dev_out, total, -(int32_t)p.n_spins);
+    count_launch(1);
     dim3 grid(p.n_words, p.n_instances, (p.n_spins + EN_CHUNK - 1) / EN_CHUNK);
     k_energy_acc<<<grid, EN_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, dev_out);
+    count_launch(1);
     return (int)cudaGetLastError();
 }
 
@@ -799,9 +807,11 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
         if (g.CW == 2) {
             XS_CU(cudaFuncSetAttribute(k_sweep_tile<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.total));
             k_sweep_tile<2><<<g.ctas, g.threads, s.total, st>>>(A);
+            count_launch(1);
         } else {
             XS_CU(cudaFuncSetAttribute(k_sweep_tile<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.total));
             k_sweep_tile<1><<<g.ctas, g.threads, s.total, st>>>(A);
+            count_launch(1);
         }
         return (int)cudaGetLastError();
     }
@@ -820,15 +830,18 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
             else
                 k_stream_set<1><<<grid, ST_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, set, s,
                                                              p.w1_threshold, p.flags, cur);
+            count_launch(1);
         }
         k_stream_commit<<<grid_for(clones, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, cur,
                                                               det[(s + 1) & 1], s, p.flags);
+        count_launch(1);
         XS_CU(cudaGetLastError());
     }
     int rc = launch_unsat_or(b, st);
     if (rc) return rc;
     k_mark_swept<<<grid_for(clones, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, b.d.det,
                                                        n_sweeps, p.flags);
+    count_launch(1);
     return (int)cudaGetLastError();
 }
 
