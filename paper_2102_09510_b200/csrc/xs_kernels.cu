@@ -23,99 +23,10 @@
 #include <cstdio>
 #include <cstdlib>
 
+#include "xs_device.cuh"
 #include "xs_internal.h"
 
 namespace xs {
-
-// ------------------------------------------------------------------------------------------
-// device helpers
-// ------------------------------------------------------------------------------------------
-template <int LUT>
-__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c)
-{
-    uint32_t d;
-    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
-    return d;
-}
-// LUT index = a*4 + b*2 + c
-constexpr int LUT_XOR3 = 0x96;
-constexpr int LUT_MAJ = 0xE8;
-constexpr int LUT_MAJ_NOTC = 0xD4;   // maj(a, b, ~c)
-constexpr int LUT_SEL = 0xCA;        // a ? b : c
-constexpr int LUT_NZ = 0x7E;         // (a^c)|(b^c): not all equal
-constexpr int LUT_OR3 = 0xFE;
-
-// Philox4x32-10 (Salmon et al., SC'11).  ctr = (c0,c1,c2,c3), key = (k0,k1).
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                              uint32_t k0, uint32_t k1, uint32_t o[4])
-{
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const uint32_t h0 = __umulhi(0xD2511F53u, c0);
-        const uint32_t l0 = 0xD2511F53u * c0;
-        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2);
-        const uint32_t l1 = 0xCD9E8D57u * c2;
-        c0 = h1 ^ c1 ^ k0;
-        c2 = h0 ^ c3 ^ k1;
-        c1 = l1;
-        c3 = l0;
-        k0 += 0x9E3779B9u;
-        k1 += 0xBB67AE85u;
-    }
-    o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
-}
-
-// One QG update of 32 clones.  a*/b* partner words, j* coupling masks, x own word, R noise mask.
-__device__ __forceinline__ uint32_t qg_update(uint32_t a0, uint32_t b0, uint32_t j0, uint32_t a1,
-                                              uint32_t b1, uint32_t j1, uint32_t a2, uint32_t b2,
-                                              uint32_t j2, uint32_t x, uint32_t R)
-{
-    const uint32_t w0 = lop3<LUT_XOR3>(a0, b0, j0);
-    const uint32_t w1 = lop3<LUT_XOR3>(a1, b1, j1);
-    const uint32_t w2 = lop3<LUT_XOR3>(a2, b2, j2);
-    const uint32_t M = lop3<LUT_MAJ>(w0, w1, w2);
-    const uint32_t P = lop3<LUT_XOR3>(w0, w1, w2);
-    const uint32_t f = lop3<LUT_MAJ_NOTC>(M, P, x);
-    return lop3<LUT_SEL>(R, f, M);
-}
-// Bits set where the spin has k != 0 unsatisfied clauses.
-__device__ __forceinline__ uint32_t qg_nonzero_k(uint32_t a0, uint32_t b0, uint32_t j0, uint32_t a1,
-                                                 uint32_t b1, uint32_t j1, uint32_t a2, uint32_t b2,
-                                                 uint32_t j2, uint32_t x)
-{
-    const uint32_t w0 = lop3<LUT_XOR3>(a0, b0, j0);
-    const uint32_t w1 = lop3<LUT_XOR3>(a1, b1, j1);
-    const uint32_t w2 = lop3<LUT_XOR3>(a2, b2, j2);
-    const uint32_t M = lop3<LUT_MAJ>(w0, w1, w2);
-    const uint32_t P = lop3<LUT_XOR3>(w0, w1, w2);
-    return lop3<LUT_NZ>(M, P, x);
-}
-
-// CW uint64 words handled by one lane, as 2*CW uint32.
-template <int CW> struct Vec;
-template <> struct Vec<1> { uint2 v; };
-template <> struct Vec<2> { uint4 v; };
-
-template <int CW> __device__ __forceinline__ void vload(const void* p, uint32_t (&o)[2 * CW]);
-template <> __device__ __forceinline__ void vload<1>(const void* p, uint32_t (&o)[2])
-{
-    const uint2 t = *reinterpret_cast<const uint2*>(p);
-    o[0] = t.x; o[1] = t.y;
-}
-template <> __device__ __forceinline__ void vload<2>(const void* p, uint32_t (&o)[4])
-{
-    const uint4 t = *reinterpret_cast<const uint4*>(p);
-    o[0] = t.x; o[1] = t.y; o[2] = t.z; o[3] = t.w;
-}
-template <int CW> __device__ __forceinline__ void vstore(void* p, const uint32_t (&o)[2 * CW]);
-template <> __device__ __forceinline__ void vstore<1>(void* p, const uint32_t (&o)[2])
-{
-    *reinterpret_cast<uint2*>(p) = make_uint2(o[0], o[1]);
-}
-template <> __device__ __forceinline__ void vstore<2>(void* p, const uint32_t (&o)[4])
-{
-    *reinterpret_cast<uint4*>(p) = make_uint4(o[0], o[1], o[2], o[3]);
-}
 
 // ------------------------------------------------------------------------------------------
 // a-2: initial state.  word(i,w) = o0 | o1 << 32 of Philox(ctr = (i, w, 0, INIT), key = run seed)
