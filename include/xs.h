@@ -85,7 +85,7 @@ typedef struct {
     uint32_t smem_bytes;     /* dynamic shared memory per CTA                                    */
     uint32_t batch_sweeps;   /* sweeps between ground-state checks inside the kernel             */
     uint32_t n_sets_max;     /* largest number of independent sets over the instances            */
-    uint32_t _pad;
+    uint32_t variant;        /* on-chip: 0 = generic tile kernel, 1 = static-task kernel         */
 } xs_layout;
 
 /* Bytes of device workspace a batch with these parameters needs (state, first-hit table,

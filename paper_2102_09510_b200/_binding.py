@@ -32,7 +32,7 @@ class xs_tts_rec(C.Structure):
 class xs_layout(C.Structure):
     _fields_ = [("regime", C.c_uint32), ("tile_words", C.c_uint32), ("threads", C.c_uint32),
                 ("ctas", C.c_uint32), ("smem_bytes", C.c_uint32), ("batch_sweeps", C.c_uint32),
-                ("n_sets_max", C.c_uint32), ("_pad", C.c_uint32)]
+                ("n_sets_max", C.c_uint32), ("variant", C.c_uint32)]
 
 
 EXPORTS = ["xs_workspace_bytes", "xs_create_instance", "xs_create_instance_from_arrays",

@@ -8,7 +8,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libxs_b200.so")
-SOURCES = ["xs_api.cu", "xs_kernels.cu", "xs_diag.cu", "xs_graph.cpp", "xs_stats.cpp"]
+SOURCES = ["xs_api.cu", "xs_kernels.cu", "xs_sweep_static.cu", "xs_diag.cu", "xs_graph.cpp", "xs_stats.cpp"]
 HEADERS = ["xs_internal.h", "xs_device.cuh", os.path.join("..", "..", "include", "xs.h")]
 
 

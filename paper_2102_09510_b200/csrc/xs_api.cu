@@ -314,7 +314,7 @@ int xs_get_layout(const xs_batch* b, xs_layout* out)
     out->smem_bytes = b->geom.smem;
     out->batch_sweeps = b->geom.batch;
     out->n_sets_max = b->n_sets_max;
-    out->_pad = 0;
+    out->variant = b->geom.variant;
     return XS_OK;
 }
 

@@ -76,7 +76,7 @@ struct TileGeom {
     uint32_t smem = 0;
     uint32_t batch = 0;        // sweeps between in-kernel ground-state checks
     uint32_t rb = 0;           // sweeps of random bytes produced at a time
-    uint32_t variant = 0;
+    uint32_t variant = 0;      // 0 generic tile kernel, 1 static-task kernel
 };
 
 }  // namespace xs
@@ -102,4 +102,9 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream);
 int launch_finalize(const xs_batch& b, uint32_t n_sweeps, void* stream);
 int launch_energy(const xs_batch& b, int32_t* dev_out, void* stream);
 bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err);
+// static-task variant (xs_sweep_static.cu)
+bool static_feasible(const xs_batch& b, uint32_t T, uint32_t threads);
+uint32_t static_rounds(const xs_batch& b, uint32_t T, uint32_t threads);
+uint32_t static_smem_bytes(uint32_t N, uint32_t T);
+int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream);
 }  // namespace xs

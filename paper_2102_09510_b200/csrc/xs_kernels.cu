@@ -593,6 +593,39 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     const uint32_t force_T = env_u32("XS_TILE_WORDS", 0);
     uint32_t bestT = 0;
     uint64_t best_cost = ~0ull;
+    // 1) static-task kernel (xs_sweep_static.cu): work list in registers, T in {8,16,32,64}
+    const uint32_t want_variant = env_u32("XS_VARIANT", 1);
+    if (!(p.flags & XS_FLAG_STREAMING) && want_variant == 1) {
+        const uint32_t force_thr = env_u32("XS_THREADS", 0);
+        uint32_t sT = 0, sThr = 0;
+        uint64_t s_cost = ~0ull;
+        for (uint32_t T = 64; T >= 8; T >>= 1) {
+            if (force_T && T != force_T) continue;
+            for (uint32_t thr = 128; thr <= 512; thr *= 2) {
+                if (force_thr && thr != force_thr) continue;
+                if (!static_feasible(b, T, thr)) continue;
+                const uint32_t smem = static_smem_bytes(p.n_spins, T);
+                const uint64_t ctas = (uint64_t)p.n_instances * (p.n_words / T);
+                const uint32_t occ = std::max(1u, std::min(SMEM_MAX / smem, 512u / thr));
+                const uint64_t waves = (ctas + (uint64_t)NUM_SMS * occ - 1) / ((uint64_t)NUM_SMS * occ);
+                // per-SM work of a wave ~ occ * T columns; few rounds = less barrier latency
+                const uint64_t cost = waves * occ * T * 16 + static_rounds(b, T, thr);
+                if (cost < s_cost) { s_cost = cost; sT = T; sThr = thr; }
+            }
+        }
+        if (sT) {
+            g.regime = 0;
+            g.variant = 1;
+            g.T = sT;
+            g.CW = 2;
+            g.threads = sThr;
+            g.ctas = p.n_instances * (p.n_words / sT);
+            g.smem = static_smem_bytes(p.n_spins, sT);
+            g.rb = 0;
+            return true;
+        }
+    }
+    // 2) generic tile kernel
     if (!(p.flags & XS_FLAG_STREAMING) && (uint64_t)p.n_spins * 8 < SMEM_MAX) {
         for (uint32_t T = 64; T >= 1; T >>= 1) {
             if (p.n_words % T) continue;
@@ -708,6 +741,7 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
     const TileGeom& g = b.geom;
     cudaStream_t st = (cudaStream_t)stream;
     if (n_sweeps == 0) return 0;
+    if (g.regime == 0 && g.variant == 1) return launch_sweep_static(b, n_sweeps, stream);
     if (g.regime == 0) {
         const TileSmem s = tile_smem(p.n_spins, g.T, g.rb, b.n_sets_max);
         TileArgs A;

@@ -87,12 +87,16 @@ def test_init_state_and_energy():
     (70, 64, 12, 64),
     (512, 32, 8, 32),     # config-3 tile shape
 ])
-def test_sweep_parity_all_words(N, W, sweeps, tile):
+@pytest.mark.parametrize("variant", [0, 1])
+def test_sweep_parity_all_words(N, W, sweeps, tile, variant):
+    """variant 0 = generic tile kernel, 1 = static-task kernel (falls back to 0 when T < 8)."""
     xs = _xs()
-    with env(XS_TILE_WORDS=tile, XS_BATCH=16):
+    with env(XS_TILE_WORDS=tile, XS_BATCH=16, XS_VARIANT=variant):
         b = xs.Batch(N, W, [N + 7], [3 * N + 1], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
     if tile:
         assert b.layout().tile_words == tile and b.layout().regime == 0
+        if variant == 0:
+            assert b.layout().variant == 0
     o = OracleRun(N, W, N + 7, 3 * N + 1, no_skip=True)
     half = sweeps // 3
     for n in (half, sweeps - half):          # two calls: resume must be exact
@@ -129,14 +133,18 @@ def test_config1_until_solved_matches_oracle_and_survey_hint(golden):
 
 @pytest.mark.parametrize("batch", [1, 5, 64])
 @pytest.mark.parametrize("streaming", [False, True])
-def test_first_hit_exact_many_solved_clones(batch, streaming):
-    """Small N: clones solve all the time -> exercises the in-kernel replay at every batch."""
+@pytest.mark.parametrize("W", [4, 8])
+def test_first_hit_exact_many_solved_clones(batch, streaming, W):
+    """Small N: clones solve all the time -> exercises the in-kernel replay at every batch.
+    W = 4 runs the generic tile kernel, W = 8 the static-task kernel (T = 8, two row copies)."""
     xs = _xs()
-    N, W = 18, 4
+    N = 18
     flags = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_STREAMING if streaming else 0)
     with env(XS_BATCH=batch):
         b = xs.Batch(N, W, [5], [9], flags=flags)
     assert b.layout().regime == (1 if streaming else 0)
+    if not streaming:
+        assert b.layout().variant == (1 if W == 8 else 0)
     o = OracleRun(N, W, 5, 9, no_skip=True)
     for n in (1, 7, 30, 13):
         b.run_sweeps(n)
