@@ -103,8 +103,8 @@ int launch_finalize(const xs_batch& b, uint32_t n_sweeps, void* stream);
 int launch_energy(const xs_batch& b, int32_t* dev_out, void* stream);
 bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err);
 // static-task variant (xs_sweep_static.cu)
-bool static_feasible(const xs_batch& b, uint32_t T, uint32_t threads);
-uint32_t static_rounds(const xs_batch& b, uint32_t T, uint32_t threads);
+bool static_feasible(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t threads);
+uint32_t static_rounds(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t threads);
 uint32_t static_smem_bytes(uint32_t N, uint32_t T);
 int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream);
 }  // namespace xs

@@ -597,27 +597,31 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     const uint32_t want_variant = env_u32("XS_VARIANT", 1);
     if (!(p.flags & XS_FLAG_STREAMING) && want_variant == 1) {
         const uint32_t force_thr = env_u32("XS_THREADS", 0);
-        uint32_t sT = 0, sThr = 0;
+        const uint32_t force_cw = env_u32("XS_CW", 0);
+        uint32_t sT = 0, sThr = 0, sCW = 0;
         uint64_t s_cost = ~0ull;
         for (uint32_t T = 64; T >= 8; T >>= 1) {
             if (force_T && T != force_T) continue;
-            for (uint32_t thr = 128; thr <= 512; thr *= 2) {
-                if (force_thr && thr != force_thr) continue;
-                if (!static_feasible(b, T, thr)) continue;
-                const uint32_t smem = static_smem_bytes(p.n_spins, T);
-                const uint64_t ctas = (uint64_t)p.n_instances * (p.n_words / T);
-                const uint32_t occ = std::max(1u, std::min(SMEM_MAX / smem, 512u / thr));
-                const uint64_t waves = (ctas + (uint64_t)NUM_SMS * occ - 1) / ((uint64_t)NUM_SMS * occ);
-                // per-SM work of a wave ~ occ * T columns; few rounds = less barrier latency
-                const uint64_t cost = waves * occ * T * 16 + static_rounds(b, T, thr);
-                if (cost < s_cost) { s_cost = cost; sT = T; sThr = thr; }
+            for (uint32_t cw = 2; cw >= 1; --cw) {
+                if (force_cw && cw != force_cw) continue;
+                for (uint32_t thr = 128; thr <= 512; thr *= 2) {
+                    if (force_thr && thr != force_thr) continue;
+                    if (!static_feasible(b, T, cw, thr)) continue;
+                    const uint32_t smem = static_smem_bytes(p.n_spins, T);
+                    const uint64_t ctas = (uint64_t)p.n_instances * (p.n_words / T);
+                    const uint32_t occ = std::max(1u, std::min(SMEM_MAX / smem, 512u / thr));
+                    const uint64_t waves = (ctas + (uint64_t)NUM_SMS * occ - 1) / ((uint64_t)NUM_SMS * occ);
+                    // per-SM work of a wave ~ occ * T columns; few rounds = less barrier latency
+                    const uint64_t cost = waves * occ * T * 16 + static_rounds(b, T, cw, thr);
+                    if (cost < s_cost) { s_cost = cost; sT = T; sThr = thr; sCW = cw; }
+                }
             }
         }
         if (sT) {
             g.regime = 0;
             g.variant = 1;
             g.T = sT;
-            g.CW = 2;
+            g.CW = sCW;
             g.threads = sThr;
             g.ctas = p.n_instances * (p.n_words / sT);
             g.smem = static_smem_bytes(p.n_spins, sT);

@@ -4,23 +4,27 @@
 // memory for the whole call; lanes <-> clone words of one spin row, sets
 // separated by __syncthreads, L277), but the work list of every thread is fixed for the whole
 // call and lives in REGISTERS: in "round" r of a sweep, thread (slot, j) updates words
-// 2j, 2j+1 of the spin at position set_start[s(r)] + q(r) * n_slots + slot.  Because the
-// update order is instance data (L289), the 7 shared-memory addresses and the 3 coupling masks
-// of each round are loaded once; the hot loop has no index loads and no address arithmetic.
+// CW*j .. CW*j+CW-1 of the spin at position set_start[s(r)] + q(r) * n_slots + slot.  Because
+// the update order is instance data (L289), the 6 partner addresses, the 3 coupling masks and
+// the thread's own spin words of each round stay in registers; the hot loop has no index
+// loads, no address arithmetic and never re-reads its own row.
 //
 // Noise (a-6): each Philox4x32-10 call yields the numbers of 4 consecutive words of a spin.
-// The two lanes (j, j^1) that share a word group compute the calls of the even and the odd
-// sweep of a sweep pair and exchange the 4 threshold bytes by one warp shuffle, so every call
-// is evaluated exactly once and nothing goes through shared memory.
+// The NL = 4 / CW lanes that share a word group each compute the call of one sweep of a period
+// of NL sweeps and exchange the threshold bytes by warp shuffles, so every call is evaluated
+// exactly once and nothing goes through shared memory.
 //
-// Bank conflicts: for T = 8 a spin row is 64 B, so the two spins served by one quarter-warp
-// phase of an LDS.128 collide when their rows have the same parity.  DUP keeps two copies of
+// Bank conflicts: for T = 8 a spin row is 64 B, so the two spins served by one 128-byte phase
+// of a shared load collide when their rows have the same parity.  DUP keeps two copies of
 // every row in one 128 B line (banks 0-15 and 16-31); even slots read copy 0, odd slots copy
 // 1, and a write updates both copies in two conflict-free stores.  T >= 16 rows are whole
-// 128 B lines and need no copy.
+// 128 B lines and need no copy.  Lanes without a task in a round work on a scratch line, so
+// the hot loop has no per-lane branch.
 //
 // Ground-state detection / exact first hit: as in k_sweep_tile (detection pass every `batch`
 // sweeps, replay of the batch from the global copy with a pass after every sweep, L293).
+#include <algorithm>
+
 #include "xs_device.cuh"
 #include "xs_internal.h"
 
@@ -35,15 +39,26 @@ struct StaticArgs {
     uint32_t off_misc;     // byte offset of det32 / known32 / flag in dynamic shared memory
 };
 
-__device__ __forceinline__ void lds128(uint32_t addr, uint32_t (&o)[4])
+// CW uint64 words = 2*CW uint32 per lane, by 32-bit shared address
+template <int CW> __device__ __forceinline__ void lds(uint32_t addr, uint32_t (&o)[2 * CW]);
+template <> __device__ __forceinline__ void lds<2>(uint32_t addr, uint32_t (&o)[4])
 {
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];"
                  : "=r"(o[0]), "=r"(o[1]), "=r"(o[2]), "=r"(o[3]) : "r"(addr) : "memory");
 }
-__device__ __forceinline__ void sts128(uint32_t addr, const uint32_t (&o)[4])
+template <> __device__ __forceinline__ void lds<1>(uint32_t addr, uint32_t (&o)[2])
+{
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(o[0]), "=r"(o[1]) : "r"(addr) : "memory");
+}
+template <int CW> __device__ __forceinline__ void sts(uint32_t addr, const uint32_t (&o)[2 * CW]);
+template <> __device__ __forceinline__ void sts<2>(uint32_t addr, const uint32_t (&o)[4])
 {
     asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};"
                  :: "r"(addr), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]) : "memory");
+}
+template <> __device__ __forceinline__ void sts<1>(uint32_t addr, const uint32_t (&o)[2])
+{
+    asm volatile("st.shared.v2.u32 [%0], {%1,%2};" :: "r"(addr), "r"(o[0]), "r"(o[1]) : "memory");
 }
 __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel)
 {
@@ -53,20 +68,25 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel)
 }
 
 // Per-round register state of a thread.
-template <int MAXT>
+template <int MAXT, int CW>
 struct Tasks {
-    uint32_t a[MAXT][6];   // shared addresses of the partner words (incl. lane and copy offset)
-    uint32_t self[MAXT];   // shared address of the own words (copy read by this thread)
-    uint32_t jm[MAXT][3];  // coupling masks
-    uint32_t rm[MAXT];     // noise: byte 2h+c = 0xFF iff word c flips k=1 spins in sweep h of the pair
-    uint32_t act;          // bit r: this thread has a task in round r
-    uint32_t bar;          // bit r: round r is the last of its set (CTA-uniform)
-    uint32_t n_rounds;     // CTA-uniform
+    uint32_t a[MAXT][6];       // shared addresses of the partner words (incl. lane and copy offset)
+    uint32_t self[MAXT];       // shared address of the own words (copy read by this thread)
+    uint32_t jm[MAXT][3];      // coupling masks
+    uint32_t rm[MAXT];         // noise bytes of the current period: byte CW*h + c = 0xFF iff word c
+                               // flips k=1 spins in sweep h of the period
+    uint32_t x[MAXT][2 * CW];  // the thread's own spin words (mirror of shared memory)
+    uint32_t act;              // bit r: this thread has a task in round r
+    uint32_t wact;             // bit r: some lane of this warp has a task in round r
+    uint32_t bar;              // bit r: round r is the last of its set (CTA-uniform)
+    uint32_t n_rounds;         // CTA-uniform
 };
 
-template <int MAXT, bool DUP, int MAXTHREADS>
+template <int MAXT, int CW, bool DUP, int MAXTHREADS>
 __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
 {
+    constexpr int H = 2 * CW;          // uint32 halves per lane
+    constexpr uint32_t NL = 4 / CW;    // lanes sharing a Philox call = sweeps per noise period
     extern __shared__ __align__(128) unsigned char smem[];
     const uint32_t N = A.N, W = A.W, T = A.T;
     const uint32_t tiles = W / T;
@@ -81,11 +101,11 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
     uint32_t* known32 = det32 + 2 * T;
     uint32_t* flag = known32 + 2 * T;
 
-    const uint32_t LPS = T / 2;
+    const uint32_t LPS = T / CW;
     const uint32_t slot = threadIdx.x / LPS, n_slots = blockDim.x / LPS;
     const uint32_t j = threadIdx.x % LPS;
     const uint32_t cpy = DUP ? (slot & 1u) * 64u : 0u;
-    const uint32_t lane_off = base + cpy + j * 16u;
+    const uint32_t lane_off = base + cpy + j * (8u * CW);
 
     const uint64_t seed = A.d.run_seed[inst];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
@@ -93,8 +113,8 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
     uint32_t* fhg = A.d.first_hit + ((size_t)inst * W + w0) * 64;
 
     // ---- static task list (a-1 tables -> registers) ---------------------------------------
-    Tasks<MAXT> tk;
-    tk.act = 0; tk.bar = 0; tk.n_rounds = 0;
+    Tasks<MAXT, CW> tk;
+    tk.act = 0; tk.wact = 0; tk.bar = 0; tk.n_rounds = 0;
     {
         const AdjRec* adj = A.d.adj + (size_t)inst * N;
         const uint32_t* ss = A.d.set_start + (size_t)inst * (N + 1);
@@ -107,7 +127,9 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
             const uint32_t pos = p0 + q * n_slots + slot;
             const bool active = valid && pos < p1;
             const bool last = valid && (p0 + (q + 1) * n_slots >= p1);
-            uint4 r0 = make_uint4(0, 0, 0, 0), r1 = make_uint4(0, 0, 0, 0);
+            // lanes without a task work on the scratch line N: no per-lane branch in the hot loop
+            uint4 r0 = make_uint4(N, N, N, N), r1 = make_uint4(N, N, N, 0);
+            if (__ballot_sync(0xFFFFFFFFu, active)) tk.wact |= 1u << r;
             if (active) {
                 const uint4* rp = reinterpret_cast<const uint4*>(adj + pos);
                 r0 = rp[0];
@@ -145,6 +167,10 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
             xg[(size_t)i * W + lw] = reinterpret_cast<const uint64_t*>(smem + ((size_t)i << shift))[lw];
         }
     };
+    auto reload_x = [&]() {
+#pragma unroll
+        for (int r = 0; r < MAXT; ++r) lds<CW>(tk.self[r], tk.x[r]);
+    };
     load_state();
     for (uint32_t e = threadIdx.x; e < 64 * T; e += blockDim.x) {
         const bool kn = fhg[e] != XS_NO_HIT;
@@ -152,48 +178,64 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
         if ((threadIdx.x & 31) == 0) known32[e >> 5] = m;
     }
     __syncthreads();
+    reload_x();
 
-    // ---- noise of sweep pair q: sweeps 2q (h = 0) and 2q + 1 (h = 1) ----------------------
-    const uint32_t grp = (w0 >> 2) + (j >> 1);
-    const uint32_t selj = (j & 1u) ? 0x3276u : 0x5410u;
+    // ---- noise of period q: sweeps NL*q + h, h = 0..NL-1 ---------------------------------
+    const uint32_t grp = (w0 + CW * j) >> 2;              // Philox word group of this lane
+    const uint32_t jl = j % NL;                           // which sweep of the period this lane computes
+    const uint32_t sub = (CW * j) & 3u;                   // first byte of this lane's words in a call
+    const int lane_base = (int)(threadIdx.x & 31u) - (int)jl;
     auto produce = [&](uint32_t q) {
-        const uint32_t t_mine = 2u * q + (j & 1u);
+        const uint32_t t_mine = NL * q + jl;
 #pragma unroll
         for (int r = 0; r < MAXT; ++r) {
             if (r < (int)tk.n_rounds) {
                 uint32_t v = 0;
-                if ((tk.act >> r) & 1u) {
+                if ((tk.wact >> r) & 1u) {
                     const uint32_t spin = (tk.self[r] - lane_off) >> shift;
                     uint32_t o[4];
                     philox4x32_10(spin, grp, t_mine, TAG_SWEEP, k0, k1, o);
                     v = (o[0] < A.thr ? 0xFFu : 0u) | (o[1] < A.thr ? 0xFF00u : 0u) |
                         (o[2] < A.thr ? 0xFF0000u : 0u) | (o[3] < A.thr ? 0xFF000000u : 0u);
                 }
-                const uint32_t other = __shfl_xor_sync(0xFFFFFFFFu, v, 1);
-                tk.rm[r] = prmt(v, other, selj);
+                if (CW == 2) {
+                    const uint32_t s0 = __shfl_sync(0xFFFFFFFFu, v, lane_base);
+                    const uint32_t s1 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 1);
+                    tk.rm[r] = prmt(s0, s1, sub ? 0x7632u : 0x5410u);
+                } else {
+                    const uint32_t s0 = __shfl_sync(0xFFFFFFFFu, v, lane_base);
+                    const uint32_t s1 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 1);
+                    const uint32_t s2 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 2);
+                    const uint32_t s3 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 3);
+                    const uint32_t pick = sub | ((4u + sub) << 4);
+                    tk.rm[r] = prmt(prmt(s0, s1, pick), prmt(s2, s3, pick), 0x5410u);
+                }
             }
         }
     };
 
-    // ---- one sweep (a-4..a-8); h selects the sweep of the pair -----------------------------
+    // ---- one sweep (a-4..a-8); h = index of the sweep inside the noise period -------------
     auto sweep = [&](uint32_t h) {
-        const uint32_t sel0 = 0x8888u + 0x2222u * h, sel1 = sel0 + 0x1111u;
+        const uint32_t sel0 = 0x8888u + 0x1111u * (CW * h);
 #pragma unroll
         for (int r = 0; r < MAXT; ++r) {
             if (r < (int)tk.n_rounds) {
-                if ((tk.act >> r) & 1u) {
-                    uint32_t a0[4], b0[4], a1[4], b1[4], a2[4], b2[4], x[4], xn[4];
-                    lds128(tk.a[r][0], a0); lds128(tk.a[r][1], b0);
-                    lds128(tk.a[r][2], a1); lds128(tk.a[r][3], b1);
-                    lds128(tk.a[r][4], a2); lds128(tk.a[r][5], b2);
-                    lds128(tk.self[r], x);
-                    const uint32_t R0 = prmt(tk.rm[r], 0u, sel0), R1 = prmt(tk.rm[r], 0u, sel1);
+                if ((tk.wact >> r) & 1u) {
+                    uint32_t a0[H], b0[H], a1[H], b1[H], a2[H], b2[H], xn[H];
+                    lds<CW>(tk.a[r][0], a0); lds<CW>(tk.a[r][1], b0);
+                    lds<CW>(tk.a[r][2], a1); lds<CW>(tk.a[r][3], b1);
+                    lds<CW>(tk.a[r][4], a2); lds<CW>(tk.a[r][5], b2);
+                    uint32_t R[CW];
 #pragma unroll
-                    for (int c = 0; c < 4; ++c)
+                    for (int c = 0; c < CW; ++c) R[c] = prmt(tk.rm[r], 0u, sel0 + 0x1111u * c);
+#pragma unroll
+                    for (int c = 0; c < H; ++c)
                         xn[c] = qg_update(a0[c], b0[c], tk.jm[r][0], a1[c], b1[c], tk.jm[r][1], a2[c],
-                                          b2[c], tk.jm[r][2], x[c], c < 2 ? R0 : R1);
-                    sts128(tk.self[r], xn);
-                    if (DUP) sts128(tk.self[r] ^ 64u, xn);
+                                          b2[c], tk.jm[r][2], tk.x[r][c], R[c >> 1]);
+                    sts<CW>(tk.self[r], xn);
+                    if (DUP) sts<CW>(tk.self[r] ^ 64u, xn);
+#pragma unroll
+                    for (int c = 0; c < H; ++c) tk.x[r][c] = xn[c];
                 }
                 if ((tk.bar >> r) & 1u) __syncthreads();
             }
@@ -205,34 +247,35 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
         for (uint32_t e = threadIdx.x; e < 2 * T; e += blockDim.x) det32[e] = 0;
         if (threadIdx.x == 0) *flag = 0;
         __syncthreads();
-        uint32_t acc[4] = {0, 0, 0, 0};
+        uint32_t acc[H];
+#pragma unroll
+        for (int c = 0; c < H; ++c) acc[c] = 0;
 #pragma unroll
         for (int r = 0; r < MAXT; ++r) {
             if (r < (int)tk.n_rounds && ((tk.act >> r) & 1u)) {
-                uint32_t a0[4], b0[4], a1[4], b1[4], a2[4], b2[4], x[4];
-                lds128(tk.a[r][0], a0); lds128(tk.a[r][1], b0);
-                lds128(tk.a[r][2], a1); lds128(tk.a[r][3], b1);
-                lds128(tk.a[r][4], a2); lds128(tk.a[r][5], b2);
-                lds128(tk.self[r], x);
+                uint32_t a0[H], b0[H], a1[H], b1[H], a2[H], b2[H];
+                lds<CW>(tk.a[r][0], a0); lds<CW>(tk.a[r][1], b0);
+                lds<CW>(tk.a[r][2], a1); lds<CW>(tk.a[r][3], b1);
+                lds<CW>(tk.a[r][4], a2); lds<CW>(tk.a[r][5], b2);
 #pragma unroll
-                for (int c = 0; c < 4; ++c)
+                for (int c = 0; c < H; ++c)
                     acc[c] |= qg_nonzero_k(a0[c], b0[c], tk.jm[r][0], a1[c], b1[c], tk.jm[r][1], a2[c],
-                                           b2[c], tk.jm[r][2], x[c]);
+                                           b2[c], tk.jm[r][2], tk.x[r][c]);
             }
         }
 #pragma unroll
-        for (int c = 0; c < 4; ++c)
-            if (acc[c]) atomicOr(&det32[4 * j + c], acc[c]);
+        for (int c = 0; c < H; ++c)
+            if (acc[c]) atomicOr(&det32[H * j + c], acc[c]);
         __syncthreads();
     };
 
     // sweeps t0+1 .. t0+n; exact: record first hits after every sweep
     auto run_range = [&](uint32_t t0, uint32_t n, bool exact) {
         const uint32_t t_first = t0 + 1, t_last = t0 + n;
-        for (uint32_t q = t_first >> 1; q <= (t_last >> 1); ++q) {
+        for (uint32_t q = t_first / NL; q <= t_last / NL; ++q) {
             produce(q);
-            for (uint32_t h = 0; h < 2; ++h) {
-                const uint32_t t = 2u * q + h;
+            for (uint32_t h = 0; h < NL; ++h) {
+                const uint32_t t = NL * q + h;
                 if (t < t_first || t > t_last) continue;
                 sweep(h);
                 if (exact) {
@@ -266,6 +309,7 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
         if (replay) {
             load_state();          // global copy = state at the start of this batch
             __syncthreads();
+            reload_x();
             run_range(t, nb, true);
         }
         store_state();             // a-10 (also the replay checkpoint of the next batch)
@@ -289,15 +333,15 @@ static uint32_t static_line_shift(uint32_t T)
 
 uint32_t static_smem_bytes(uint32_t N, uint32_t T)
 {
-    const uint64_t state = (uint64_t)N << static_line_shift(T);
+    const uint64_t state = ((uint64_t)N + 1) << static_line_shift(T);   // + scratch line
     const uint64_t total = state + (4ull * T + 4) * 4 + 128;
     return total > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)total;
 }
 
 // rounds a CTA of `threads` threads needs per sweep for tile width T (max over instances)
-uint32_t static_rounds(const xs_batch& b, uint32_t T, uint32_t threads)
+uint32_t static_rounds(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t threads)
 {
-    const uint32_t n_slots = threads / (T / 2);
+    const uint32_t n_slots = threads / (T / CW);
     if (n_slots == 0) return 0xFFFFFFFFu;
     uint32_t worst = 0;
     for (const HostGraph& g : b.graphs) {
@@ -309,12 +353,35 @@ uint32_t static_rounds(const xs_batch& b, uint32_t T, uint32_t threads)
     return worst;
 }
 
-bool static_feasible(const xs_batch& b, uint32_t T, uint32_t threads)
+bool static_feasible(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t threads)
 {
     if (T < 8 || T > 64 || (T & (T - 1)) || b.p.n_words % T) return false;
-    if (threads % 32 || threads < 32 || threads > 512 || threads % (T / 2)) return false;
+    if (CW != 1 && CW != 2) return false;
+    const uint32_t LPS = T / CW;
+    if (LPS > 32) return false;
+    if (threads % 32 || threads < 32 || threads > 512 || threads % LPS) return false;
     if (static_smem_bytes(b.p.n_spins, T) > STATIC_SMEM_MAX) return false;
-    return static_rounds(b, T, threads) <= (uint32_t)STATIC_MAXT;
+    return static_rounds(b, T, CW, threads) <= (uint32_t)STATIC_MAXT;
+}
+
+template <int MAXT, int CW, bool DUP, int MT>
+static cudaError_t launch_k(const StaticArgs& A, uint32_t ctas, uint32_t threads, uint32_t smem,
+                            cudaStream_t st)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_static<MAXT, CW, DUP, MT>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_sweep_static<MAXT, CW, DUP, MT><<<ctas, threads, smem, st>>>(A);
+    return cudaGetLastError();
+}
+static uint32_t g_rounds_for_launch = STATIC_MAXT;
+template <int CW, bool DUP, int MT>
+static cudaError_t launch_one(const StaticArgs& A, uint32_t ctas, uint32_t threads, uint32_t smem,
+                              cudaStream_t st)
+{
+    // fewer unrolled rounds = fewer registers (the 512-thread variants are capped at 128)
+    if (g_rounds_for_launch <= 6) return launch_k<6, CW, DUP, MT>(A, ctas, threads, smem, st);
+    return launch_k<STATIC_MAXT, CW, DUP, MT>(A, ctas, threads, smem, st);
 }
 
 int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream)
@@ -326,25 +393,25 @@ int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream)
     A.N = p.n_spins; A.W = p.n_words; A.T = g.T; A.n_sweeps = n_sweeps;
     A.thr = p.w1_threshold; A.flags = p.flags; A.batch = g.batch;
     A.line_shift = static_line_shift(g.T);
-    A.off_misc = (uint32_t)(((uint64_t)p.n_spins << A.line_shift) + 127) / 128 * 128;
-    const uint32_t smem = g.smem;
+    A.off_misc = (uint32_t)((((uint64_t)p.n_spins + 1) << A.line_shift) + 127) / 128 * 128;
     cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = cudaSuccess;
-#define XS_LAUNCH(DUPV, MT)                                                                            \
-    do {                                                                                               \
-        e = cudaFuncSetAttribute(k_sweep_static<STATIC_MAXT, DUPV, MT>,                                \
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);              \
-        if (e == cudaSuccess) k_sweep_static<STATIC_MAXT, DUPV, MT><<<g.ctas, g.threads, smem, st>>>(A); \
-    } while (0)
-    if (g.T == 8) {
-        if (g.threads <= 256) XS_LAUNCH(true, 256); else XS_LAUNCH(true, 512);
+    const bool dup = g.T == 8, small = g.threads <= 256;
+    g_rounds_for_launch = static_rounds(b, g.T, g.CW, g.threads);
+    cudaError_t e;
+    if (g.CW == 2) {
+        if (dup) e = small ? launch_one<2, true, 256>(A, g.ctas, g.threads, g.smem, st)
+                           : launch_one<2, true, 512>(A, g.ctas, g.threads, g.smem, st);
+        else     e = small ? launch_one<2, false, 256>(A, g.ctas, g.threads, g.smem, st)
+                           : launch_one<2, false, 512>(A, g.ctas, g.threads, g.smem, st);
     } else {
-        if (g.threads <= 256) XS_LAUNCH(false, 256); else XS_LAUNCH(false, 512);
+        if (dup) e = small ? launch_one<1, true, 256>(A, g.ctas, g.threads, g.smem, st)
+                           : launch_one<1, true, 512>(A, g.ctas, g.threads, g.smem, st);
+        else     e = small ? launch_one<1, false, 256>(A, g.ctas, g.threads, g.smem, st)
+                           : launch_one<1, false, 512>(A, g.ctas, g.threads, g.smem, st);
     }
-#undef XS_LAUNCH
     if (e != cudaSuccess) return (int)e;
     count_launch(1);
-    return (int)cudaGetLastError();
+    return 0;
 }
 
 }  // namespace xs

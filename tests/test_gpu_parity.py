@@ -106,6 +106,27 @@ def test_sweep_parity_all_words(N, W, sweeps, tile, variant):
     b.close()
 
 
+@pytest.mark.parametrize("N,W,tile,threads,sweeps", [
+    (256, 8, 8, 512, 37),     # config-2 tile, one uint64 word per lane, two row copies
+    (100, 16, 16, 512, 23),
+    (60, 32, 32, 512, 21),
+    (18, 8, 8, 128, 45),      # many solved clones: replay path with a 4-sweep noise period
+])
+def test_static_kernel_one_word_per_lane(N, W, tile, threads, sweeps):
+    """Static-task kernel with CW = 1: four lanes share a Philox call over a 4-sweep period."""
+    xs = _xs()
+    with env(XS_TILE_WORDS=tile, XS_BATCH=10, XS_VARIANT=1, XS_CW=1, XS_THREADS=threads):
+        b = xs.Batch(N, W, [N + 3], [N + 4], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
+    lay = b.layout()
+    assert (lay.variant, lay.tile_words, lay.threads) == (1, tile, threads)
+    o = OracleRun(N, W, N + 3, N + 4, no_skip=True)
+    for n in (1, 2, 3, sweeps - 6):
+        b.run_sweeps(n)
+        o.run_sweeps(n)
+        _compare(b, [o], f"CW=1 N={N} W={W}")
+    b.close()
+
+
 def test_config1_until_solved_matches_oracle_and_survey_hint(golden):
     """BASELINE.json configs[0]: N=64, seed 1, 64 clones, until E=-N, K=100 sweeps per call."""
     xs = _xs()
