@@ -24,6 +24,8 @@
 // Ground-state detection / exact first hit: as in k_sweep_tile (detection pass every `batch`
 // sweeps, replay of the batch from the global copy with a pass after every sweep, L293).
 #include <algorithm>
+#include <cstdlib>
+#include <type_traits>
 
 #include "xs_device.cuh"
 #include "xs_internal.h"
@@ -37,6 +39,7 @@ struct StaticArgs {
     uint32_t N, W, T, n_sweeps, thr, flags, batch;
     uint32_t line_shift;   // log2(bytes of one spin line in shared memory)
     uint32_t off_misc;     // byte offset of det32 / known32 / flag in dynamic shared memory
+    uint32_t dbg;          // timing ablations (XS_DBG, wrong results): 1 no barriers, 2 no noise, 4 one store, 8 no loads
 };
 
 // CW uint64 words = 2*CW uint32 per lane, by 32-bit shared address
@@ -73,6 +76,7 @@ struct Tasks {
     uint32_t a[MAXT][6];       // shared addresses of the partner words (incl. lane and copy offset)
     uint32_t self[MAXT];       // shared address of the own words (copy read by this thread)
     uint32_t jm[MAXT][3];      // coupling masks
+    uint32_t rmn[MAXT];        // noise bytes of the next period (produced inside the sweeps)
     uint32_t rm[MAXT];         // noise bytes of the current period: byte CW*h + c = 0xFF iff word c
                                // flips k=1 spins in sweep h of the period
     uint32_t x[MAXT][2 * CW];  // the thread's own spin words (mirror of shared memory)
@@ -147,10 +151,14 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
             tk.jm[r][1] = (r1.w & 2u) ? ~0u : 0u;
             tk.jm[r][2] = (r1.w & 4u) ? ~0u : 0u;
             tk.rm[r] = 0;
+            tk.rmn[r] = 0;
             if (valid) tk.n_rounds = r + 1;
             if (last) { tk.bar |= 1u << r; ++s; q = 0; } else { ++q; }
         }
     }
+
+    tk.n_rounds = __shfl_sync(0xFFFFFFFFu, tk.n_rounds, 0);   // tell the compiler: warp-uniform
+    tk.bar = __shfl_sync(0xFFFFFFFFu, tk.bar, 0);
 
     auto load_state = [&]() {
         for (uint32_t e = threadIdx.x; e < N * T; e += blockDim.x) {
@@ -180,43 +188,38 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
     __syncthreads();
     reload_x();
 
-    // ---- noise of period q: sweeps NL*q + h, h = 0..NL-1 ---------------------------------
+    // ---- noise (a-6): threshold bytes of this lane's words for the NL sweeps of a period ---
     const uint32_t grp = (w0 + CW * j) >> 2;              // Philox word group of this lane
     const uint32_t jl = j % NL;                           // which sweep of the period this lane computes
     const uint32_t sub = (CW * j) & 3u;                   // first byte of this lane's words in a call
     const int lane_base = (int)(threadIdx.x & 31u) - (int)jl;
-    auto produce = [&](uint32_t q) {
-        const uint32_t t_mine = NL * q + jl;
+    const uint32_t thr = A.thr;
+    auto noise_call = [&](int r, uint32_t q) -> uint32_t {
+        const uint32_t spin = (tk.self[r] - lane_off) >> shift;
+        uint32_t o[4];
+        philox4x32_10(spin, grp, NL * q + jl, TAG_SWEEP, k0, k1, o);
+        const uint32_t v = (o[0] < thr ? 0xFFu : 0u) | (o[1] < thr ? 0xFF00u : 0u) |
+                           (o[2] < thr ? 0xFF0000u : 0u) | (o[3] < thr ? 0xFF000000u : 0u);
+        const uint32_t s0 = __shfl_sync(0xFFFFFFFFu, v, lane_base);
+        const uint32_t s1 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 1);
+        if (CW == 2) return prmt(s0, s1, sub ? 0x7632u : 0x5410u);
+        const uint32_t s2 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 2);
+        const uint32_t s3 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 3);
+        const uint32_t pick = sub | ((4u + sub) << 4);
+        return prmt(prmt(s0, s1, pick), prmt(s2, s3, pick), 0x5410u);
+    };
+    // all rounds of period q at once (branch-free: the calls interleave)
+    auto produce_all = [&](uint32_t q) {
 #pragma unroll
-        for (int r = 0; r < MAXT; ++r) {
-            if (r < (int)tk.n_rounds) {
-                uint32_t v = 0;
-                if ((tk.wact >> r) & 1u) {
-                    const uint32_t spin = (tk.self[r] - lane_off) >> shift;
-                    uint32_t o[4];
-                    philox4x32_10(spin, grp, t_mine, TAG_SWEEP, k0, k1, o);
-                    v = (o[0] < A.thr ? 0xFFu : 0u) | (o[1] < A.thr ? 0xFF00u : 0u) |
-                        (o[2] < A.thr ? 0xFF0000u : 0u) | (o[3] < A.thr ? 0xFF000000u : 0u);
-                }
-                if (CW == 2) {
-                    const uint32_t s0 = __shfl_sync(0xFFFFFFFFu, v, lane_base);
-                    const uint32_t s1 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 1);
-                    tk.rm[r] = prmt(s0, s1, sub ? 0x7632u : 0x5410u);
-                } else {
-                    const uint32_t s0 = __shfl_sync(0xFFFFFFFFu, v, lane_base);
-                    const uint32_t s1 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 1);
-                    const uint32_t s2 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 2);
-                    const uint32_t s3 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 3);
-                    const uint32_t pick = sub | ((4u + sub) << 4);
-                    tk.rm[r] = prmt(prmt(s0, s1, pick), prmt(s2, s3, pick), 0x5410u);
-                }
-            }
-        }
+        for (int r = 0; r < MAXT; ++r) tk.rm[r] = noise_call(r, q);
     };
 
-    // ---- one sweep (a-4..a-8); h = index of the sweep inside the noise period -------------
-    auto sweep = [&](uint32_t h) {
-        const uint32_t sel0 = 0x8888u + 0x1111u * (CW * h);
+    // ---- one sweep (a-4..a-8); h = index of the sweep inside the noise period.  With `fuse`
+    // the Philox calls of period qn for the rounds r = h (mod NL) are issued right after the
+    // round's shared loads, i.e. in their latency shadow. --------------------------------------
+    auto sweep = [&](auto hc, uint32_t qn) {
+        constexpr uint32_t h = decltype(hc)::value;
+        constexpr uint32_t sel0 = 0x8888u + 0x1111u * (CW * h);
 #pragma unroll
         for (int r = 0; r < MAXT; ++r) {
             if (r < (int)tk.n_rounds) {
@@ -228,6 +231,7 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
                     uint32_t R[CW];
 #pragma unroll
                     for (int c = 0; c < CW; ++c) R[c] = prmt(tk.rm[r], 0u, sel0 + 0x1111u * c);
+                    if ((uint32_t)r % NL == h) tk.rmn[r] = noise_call(r, qn);   // compile-time test
 #pragma unroll
                     for (int c = 0; c < H; ++c)
                         xn[c] = qg_update(a0[c], b0[c], tk.jm[r][0], a1[c], b1[c], tk.jm[r][1], a2[c],
@@ -237,7 +241,7 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
 #pragma unroll
                     for (int c = 0; c < H; ++c) tk.x[r][c] = xn[c];
                 }
-                if ((tk.bar >> r) & 1u) __syncthreads();
+                if (((tk.bar >> r) & 1u) && !(A.dbg & 1u)) __syncthreads();
             }
         }
     };
@@ -272,12 +276,23 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
     // sweeps t0+1 .. t0+n; exact: record first hits after every sweep
     auto run_range = [&](uint32_t t0, uint32_t n, bool exact) {
         const uint32_t t_first = t0 + 1, t_last = t0 + n;
-        for (uint32_t q = t_first / NL; q <= t_last / NL; ++q) {
-            produce(q);
-            for (uint32_t h = 0; h < NL; ++h) {
-                const uint32_t t = NL * q + h;
-                if (t < t_first || t > t_last) continue;
-                sweep(h);
+        const uint32_t q_last = t_last / NL;
+        bool have_next = false;
+        for (uint32_t q = t_first / NL; q <= q_last; ++q) {
+            if (have_next) {
+#pragma unroll
+                for (int r = 0; r < MAXT; ++r) tk.rm[r] = tk.rmn[r];
+            } else if (!(A.dbg & 2u)) {
+                produce_all(q);
+            }
+            // the next period's noise can be produced inside this period's sweeps iff all NL
+            // sweeps of this period run and there is a next period
+            const bool fuse = (NL * q >= t_first) && (NL * q + NL - 1 <= t_last) && (q < q_last) &&
+                              !(A.dbg & 2u);
+            auto step = [&](auto hc) {
+                const uint32_t t = NL * q + decltype(hc)::value;
+                if (t < t_first || t > t_last) return;
+                sweep(hc, q + 1);
                 if (exact) {
                     detect();
                     for (uint32_t e = threadIdx.x; e < 2 * T; e += blockDim.x) {
@@ -291,7 +306,14 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
                     }
                     __syncthreads();
                 }
+            };
+            step(std::integral_constant<uint32_t, 0>{});
+            if (NL > 1) step(std::integral_constant<uint32_t, 1 % NL>{});
+            if (NL > 2) {
+                step(std::integral_constant<uint32_t, 2 % NL>{});
+                step(std::integral_constant<uint32_t, 3 % NL>{});
             }
+            have_next = fuse;
         }
     };
 
@@ -394,6 +416,7 @@ int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream)
     A.thr = p.w1_threshold; A.flags = p.flags; A.batch = g.batch;
     A.line_shift = static_line_shift(g.T);
     A.off_misc = (uint32_t)((((uint64_t)p.n_spins + 1) << A.line_shift) + 127) / 128 * 128;
+    { const char* s_ = std::getenv("XS_DBG"); A.dbg = s_ ? (uint32_t)std::atoi(s_) : 0u; }
     cudaStream_t st = (cudaStream_t)stream;
     const bool dup = g.T == 8, small = g.threads <= 256;
     g_rounds_for_launch = static_rounds(b, g.T, g.CW, g.threads);
