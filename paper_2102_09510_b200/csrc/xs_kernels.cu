@@ -593,9 +593,19 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     const uint32_t force_T = env_u32("XS_TILE_WORDS", 0);
     uint32_t bestT = 0;
     uint64_t best_cost = ~0ull;
+    // Measured on B200 (profiles/geometry_sweep_r01.md): with at least one 16-column tile per SM
+    // the generic kernel with T = 16 (128-byte rows: conflict-free, several CTAs per SM overlap
+    // their load / compute / barrier phases) is the fastest choice; with fewer tiles than SMs
+    // (config 2) the static-task kernel with T = 8 wins because one CTA per SM must hide its
+    // own latencies.  XS_VARIANT: unset = this rule, 0 = generic only, 1 = static if feasible.
+    const uint32_t want_variant = env_u32("XS_VARIANT", 2);
+    const bool many_tiles = (p.n_words % 16 == 0) &&
+                            (uint64_t)p.n_instances * (p.n_words / 16) >= NUM_SMS &&
+                            tile_smem(p.n_spins, 16, 1, b.n_sets_max).total <= SMEM_MAX;
+    uint32_t auto_T = 0;
+    if (want_variant == 2 && many_tiles && !force_T) auto_T = 16;
     // 1) static-task kernel (xs_sweep_static.cu): work list in registers, T in {8,16,32,64}
-    const uint32_t want_variant = env_u32("XS_VARIANT", 1);
-    if (!(p.flags & XS_FLAG_STREAMING) && want_variant == 1) {
+    if (!(p.flags & XS_FLAG_STREAMING) && (want_variant == 1 || (want_variant == 2 && !auto_T))) {
         const uint32_t force_thr = env_u32("XS_THREADS", 0);
         const uint32_t force_cw = env_u32("XS_CW", 0);
         uint32_t sT = 0, sThr = 0, sCW = 0;
@@ -609,10 +619,12 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
                     if (!static_feasible(b, T, cw, thr)) continue;
                     const uint32_t smem = static_smem_bytes(p.n_spins, T);
                     const uint64_t ctas = (uint64_t)p.n_instances * (p.n_words / T);
-                    const uint32_t occ = std::max(1u, std::min(SMEM_MAX / smem, 512u / thr));
-                    const uint64_t waves = (ctas + (uint64_t)NUM_SMS * occ - 1) / ((uint64_t)NUM_SMS * occ);
-                    // per-SM work of a wave ~ occ * T columns; few rounds = less barrier latency
-                    const uint64_t cost = waves * occ * T * 16 + static_rounds(b, T, cw, thr);
+                    if (smem > SMEM_MAX) continue;
+                    // work of the busiest SM ~ (CTAs it gets) x T columns; then fewer rounds
+                    // (= fewer barriers per sweep); 512-thread CTAs are register-capped at 128
+                    const uint64_t per_sm = (ctas + NUM_SMS - 1) / NUM_SMS;
+                    const uint64_t cost = per_sm * T * 16 + static_rounds(b, T, cw, thr) +
+                                          (thr == 512 ? 2 : 0) + (cw == 1 ? 1 : 0);
                     if (cost < s_cost) { s_cost = cost; sT = T; sThr = thr; sCW = cw; }
                 }
             }
@@ -634,6 +646,7 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
         for (uint32_t T = 64; T >= 1; T >>= 1) {
             if (p.n_words % T) continue;
             if (force_T && T != force_T) continue;
+            if (auto_T && T != auto_T) continue;
             const TileSmem s = tile_smem(p.n_spins, T, 1, b.n_sets_max);
             if (s.total > SMEM_MAX) continue;
             const uint64_t ctas = (uint64_t)p.n_instances * (p.n_words / T);
