@@ -163,7 +163,8 @@ def main():
 
     N, W, I, sweeps = wl["N"], wl["W"], wl["I"], wl["sweeps"]
     gseeds = [wl["graph_seed"] + i for i in range(I)]
-    rseeds = [wl["run_seed"] + i + 1000 * rank for i in range(I)]      # replicas: own run seeds (L87)
+    from paper_2102_09510_b200 import replicas
+    rseeds = replicas.replica_run_seeds([wl["run_seed"] + i for i in range(I)], rank)   # replicas (L87)
     b = xs.Batch(N, W, gseeds, rseeds, flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP, device=dev)
     lay = b.layout()
     updates_per_step = float(N) * 64.0 * W * I * sweeps
@@ -243,12 +244,9 @@ def main():
     barrier()
     e2e_ms = float(sum(ev[0].elapsed_time(ev[2]) for ev in evs2))
 
-    if dist is not None:
-        t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, e2e_ms = float(t[0]), float(t[1])
-    value = world * updates_per_step * args.steps / (total_ms * 1e6)
-    e2e_value = world * updates_per_step * args.steps / (e2e_ms * 1e6)
+    total_ms, e2e_ms = replicas.max_over_ranks([total_ms, e2e_ms], dist, dev)   # max over ranks
+    value = replicas.job_rate(updates_per_step, args.steps, world, total_ms)
+    e2e_value = replicas.job_rate(updates_per_step, args.steps, world, e2e_ms)
 
     if rank == 0:
         k_ms = float(np.mean(sweep_ms))

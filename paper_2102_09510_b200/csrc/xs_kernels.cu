@@ -575,7 +575,7 @@ struct TileSmem { uint32_t off_rec, off_rbuf, off_sets, off_misc, total; };
 TileSmem tile_smem(uint32_t N, uint32_t T, uint32_t rb, uint32_t n_sets_max)
 {
     TileSmem s;
-    uint64_t o = (uint64_t)N * T * 8;
+    uint64_t o = ((uint64_t)N * T * 8 + 15) / 16 * 16;   // records are read as 16-byte vectors
     s.off_rec = (uint32_t)o;           o += (uint64_t)N * 48;
     s.off_rbuf = (uint32_t)o;          o += round_up(rb * N * T, 16);
     s.off_sets = (uint32_t)o;          o += round_up((n_sets_max + 1) * 4, 16);
@@ -610,7 +610,7 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
         const uint32_t force_cw = env_u32("XS_CW", 0);
         uint32_t sT = 0, sThr = 0, sCW = 0;
         uint64_t s_cost = ~0ull;
-        for (uint32_t T = 64; T >= 8; T >>= 1) {
+        for (uint32_t T = 64; T >= 4; T >>= 1) {
             if (force_T && T != force_T) continue;
             for (uint32_t cw = 2; cw >= 1; --cw) {
                 if (force_cw && cw != force_cw) continue;

@@ -86,7 +86,7 @@ struct Tasks {
     uint32_t n_rounds;         // CTA-uniform
 };
 
-template <int MAXT, int CW, bool DUP, int MAXTHREADS>
+template <int MAXT, int CW, int NC, int MAXTHREADS>
 __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
 {
     constexpr int H = 2 * CW;          // uint32 halves per lane
@@ -108,7 +108,10 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
     const uint32_t LPS = T / CW;
     const uint32_t slot = threadIdx.x / LPS, n_slots = blockDim.x / LPS;
     const uint32_t j = threadIdx.x % LPS;
-    const uint32_t cpy = DUP ? (slot & 1u) * 64u : 0u;
+    // NC copies of every row in its 128-byte line; slot s reads copy s % NC (conflict-free phases)
+    constexpr uint32_t ROWB = 128u / NC;                  // bytes of one copy (= 8 T when NC > 1)
+    const uint32_t sm = slot % NC;
+    const uint32_t cpy = NC > 1 ? sm * ROWB : 0u;
     const uint32_t lane_off = base + cpy + j * (8u * CW);
 
     const uint64_t seed = A.d.run_seed[inst];
@@ -166,7 +169,8 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
             const uint64_t v = xg[(size_t)i * W + lw];
             unsigned char* line = smem + ((size_t)i << shift);
             reinterpret_cast<uint64_t*>(line)[lw] = v;
-            if (DUP) reinterpret_cast<uint64_t*>(line + 64)[lw] = v;
+#pragma unroll
+            for (int c = 1; c < NC; ++c) reinterpret_cast<uint64_t*>(line + c * ROWB)[lw] = v;
         }
     };
     auto store_state = [&]() {
@@ -237,7 +241,10 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
                         xn[c] = qg_update(a0[c], b0[c], tk.jm[r][0], a1[c], b1[c], tk.jm[r][1], a2[c],
                                           b2[c], tk.jm[r][2], tk.x[r][c], R[c >> 1]);
                     sts<CW>(tk.self[r], xn);
-                    if (DUP) sts<CW>(tk.self[r] ^ 64u, xn);
+                    // the other copies: in store c, slot s writes copy (s + c) % NC
+#pragma unroll
+                    for (int c = 1; c < NC; ++c)
+                        sts<CW>(tk.self[r] + (((sm + c) % NC) - sm) * ROWB, xn);
 #pragma unroll
                     for (int c = 0; c < H; ++c) tk.x[r][c] = xn[c];
                 }
@@ -348,7 +355,7 @@ constexpr uint32_t STATIC_SMEM_MAX = 227u * 1024u;
 
 static uint32_t static_line_shift(uint32_t T)
 {
-    uint32_t bytes = (T == 8) ? 128u : T * 8u, sh = 0;
+    uint32_t bytes = (T <= 16) ? 128u : T * 8u, sh = 0;   // T = 4, 8: 4 / 2 copies in one line
     while ((1u << sh) < bytes) ++sh;
     return sh;
 }
@@ -377,7 +384,7 @@ uint32_t static_rounds(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t thre
 
 bool static_feasible(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t threads)
 {
-    if (T < 8 || T > 64 || (T & (T - 1)) || b.p.n_words % T) return false;
+    if (T < 4 || T > 64 || (T & (T - 1)) || b.p.n_words % T) return false;
     if (CW != 1 && CW != 2) return false;
     const uint32_t LPS = T / CW;
     if (LPS > 32) return false;
@@ -386,24 +393,24 @@ bool static_feasible(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t thread
     return static_rounds(b, T, CW, threads) <= (uint32_t)STATIC_MAXT;
 }
 
-template <int MAXT, int CW, bool DUP, int MT>
+template <int MAXT, int CW, int NC, int MT>
 static cudaError_t launch_k(const StaticArgs& A, uint32_t ctas, uint32_t threads, uint32_t smem,
                             cudaStream_t st)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_static<MAXT, CW, DUP, MT>,
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_static<MAXT, CW, NC, MT>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_sweep_static<MAXT, CW, DUP, MT><<<ctas, threads, smem, st>>>(A);
+    k_sweep_static<MAXT, CW, NC, MT><<<ctas, threads, smem, st>>>(A);
     return cudaGetLastError();
 }
 static uint32_t g_rounds_for_launch = STATIC_MAXT;
-template <int CW, bool DUP, int MT>
+template <int CW, int NC, int MT>
 static cudaError_t launch_one(const StaticArgs& A, uint32_t ctas, uint32_t threads, uint32_t smem,
                               cudaStream_t st)
 {
     // fewer unrolled rounds = fewer registers (the 512-thread variants are capped at 128)
-    if (g_rounds_for_launch <= 6) return launch_k<6, CW, DUP, MT>(A, ctas, threads, smem, st);
-    return launch_k<STATIC_MAXT, CW, DUP, MT>(A, ctas, threads, smem, st);
+    if (g_rounds_for_launch <= 6) return launch_k<6, CW, NC, MT>(A, ctas, threads, smem, st);
+    return launch_k<STATIC_MAXT, CW, NC, MT>(A, ctas, threads, smem, st);
 }
 
 int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream)
@@ -418,20 +425,19 @@ int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream)
     A.off_misc = (uint32_t)((((uint64_t)p.n_spins + 1) << A.line_shift) + 127) / 128 * 128;
     { const char* s_ = std::getenv("XS_DBG"); A.dbg = s_ ? (uint32_t)std::atoi(s_) : 0u; }
     cudaStream_t st = (cudaStream_t)stream;
-    const bool dup = g.T == 8, small = g.threads <= 256;
+    const uint32_t nc = g.T <= 16 ? 16u / g.T : 1u;     // row copies per 128-byte line
+    const bool small = g.threads <= 256;
     g_rounds_for_launch = static_rounds(b, g.T, g.CW, g.threads);
     cudaError_t e;
+#define XS_STATIC_LAUNCH(CWV, NCV)                                                          \
+    e = small ? launch_one<CWV, NCV, 256>(A, g.ctas, g.threads, g.smem, st)                 \
+              : launch_one<CWV, NCV, 512>(A, g.ctas, g.threads, g.smem, st)
     if (g.CW == 2) {
-        if (dup) e = small ? launch_one<2, true, 256>(A, g.ctas, g.threads, g.smem, st)
-                           : launch_one<2, true, 512>(A, g.ctas, g.threads, g.smem, st);
-        else     e = small ? launch_one<2, false, 256>(A, g.ctas, g.threads, g.smem, st)
-                           : launch_one<2, false, 512>(A, g.ctas, g.threads, g.smem, st);
+        if (nc == 4) XS_STATIC_LAUNCH(2, 4); else if (nc == 2) XS_STATIC_LAUNCH(2, 2); else XS_STATIC_LAUNCH(2, 1);
     } else {
-        if (dup) e = small ? launch_one<1, true, 256>(A, g.ctas, g.threads, g.smem, st)
-                           : launch_one<1, true, 512>(A, g.ctas, g.threads, g.smem, st);
-        else     e = small ? launch_one<1, false, 256>(A, g.ctas, g.threads, g.smem, st)
-                           : launch_one<1, false, 512>(A, g.ctas, g.threads, g.smem, st);
+        if (nc == 4) XS_STATIC_LAUNCH(1, 4); else if (nc == 2) XS_STATIC_LAUNCH(1, 2); else XS_STATIC_LAUNCH(1, 1);
     }
+#undef XS_STATIC_LAUNCH
     if (e != cudaSuccess) return (int)e;
     count_launch(1);
     return 0;

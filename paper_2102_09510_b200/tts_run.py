@@ -1,0 +1,107 @@
+"""TTS accounting runs (SURVEY.md 8(a) a-12, 8(d) "TTS percentiles as the paper defines").
+
+    python -m paper_2102_09510_b200.tts_run --n 128 --words 64 --instances 256 --runs 16 --cap 200000
+
+For every instance (graph seed) R independent runs (different run seeds: "running
+the QG algorithm 1008 times") are put into one batch of instances x runs entries; the batch is
+advanced K sweeps per call (L293: ~100) until every entry is solved or the cap (timeout t_max,
+L129) is reached; entries that already have a solved clone are skipped by the library.  Per
+instance: tau_hat, model and empirical TTS_50/90/99, posterior quantiles (xs_tts_stats).  Over
+instances: the median of TTS_99 (the competition's figure) and the median tau.  Times are
+reported in sweeps (hardware free) and in seconds = sweeps x measured seconds per sweep of a run
+of this batch shape.  Only marshals calls into the C ABI; prints one JSON line per size.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import time
+
+import numpy as np
+
+
+def run_size(n, words, instances, runs, cap, chunk, seed0, flags_extra=0):
+    import torch
+    import paper_2102_09510_b200 as xs
+    gseeds = [seed0 + i for i in range(instances) for _ in range(runs)]
+    rseeds = [seed0 + i + 7919 * (r + 1) for i in range(instances) for r in range(runs)]
+    b = xs.Batch(n, words, gseeds, rseeds, flags=xs.XS_FLAG_GAUGE | flags_extra)
+    lay = b.layout()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    done = 0
+    gpu_ms = 0.0
+    t0 = time.time()
+    unsolved_sweeps = 0.0
+    while done < cap:
+        k = min(chunk, cap - done)
+        recs_before = b.tts()
+        active = sum(1 for r in recs_before if not r.solved)
+        if active == 0:
+            break
+        ev0.record()
+        b.run_sweeps(k)
+        ev1.record()
+        torch.cuda.synchronize()
+        gpu_ms += ev0.elapsed_time(ev1)
+        unsolved_sweeps += active * k
+        done += k
+    recs = b.tts()
+    tts = np.array([r.tts_sweeps for r in recs], dtype=np.uint32).reshape(instances, runs)
+    clones = 64 * words
+    sec_per_sweep = (gpu_ms * 1e-3) / max(unsolved_sweeps, 1.0)      # per batch entry
+    per_inst = [xs.xs_tts_stats(tts[i], cap) for i in range(instances)]
+    taus = np.array([s["tau_hat"] for s in per_inst])
+    tts99 = np.array([s["tts99_model"] for s in per_inst])
+    n_solved_runs = int((tts != xs.XS_NO_HIT).sum())
+    solved_inst = int(sum(1 for s in per_inst if s["n_solved"] > 0))
+    med = lambda a: float(np.median(a)) if np.isfinite(np.median(a)) else None   # noqa: E731
+    lower = [s["tau_q16"] for s in per_inst if s["n_solved"] == 0]
+    out = {
+        "n_spins": n, "clones": clones, "instances": instances, "runs_per_instance": runs,
+        "cap_sweeps": cap, "chunk": chunk, "regime": lay.regime, "tile_words": lay.tile_words,
+        "solved_runs": n_solved_runs, "total_runs": instances * runs, "instances_with_a_solved_run": solved_inst,
+        "median_tau_sweeps": med(taus), "median_tts99_sweeps": med(tts99),
+        "median_tts50_sweeps": med(np.array([s["tts50_model"] for s in per_inst])),
+        "median_tts90_sweeps": med(np.array([s["tts90_model"] for s in per_inst])),
+        "p90_over_instances_tau_sweeps": float(np.percentile(taus, 90)) if np.isfinite(np.percentile(taus, 90)) else None,
+        "hardest_decile_median_tts_sweeps": (float(np.median(np.sort(taus)[-max(1, instances // 10):]) * math.log(2))
+                                             if np.isfinite(taus).all() else None),
+        "tau_lower_bound_95_if_unsolved_sweeps": float(np.median(lower)) if lower else None,
+        "single_clone_t0_clone_sweeps": (med(taus) * clones) if med(taus) else None,
+        "sec_per_sweep_per_run": sec_per_sweep,
+        "median_tts99_seconds": (med(tts99) * sec_per_sweep) if med(tts99) else None,
+        "updates_per_ns": n * clones * unsolved_sweeps / max(gpu_ms * 1e6, 1e-9),
+        "gpu_ms": gpu_ms, "wall_s": time.time() - t0,
+    }
+    b.close()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--n", type=int, nargs="+", default=[128])
+    ap.add_argument("--words", type=int, default=64)
+    ap.add_argument("--instances", type=int, default=256)
+    ap.add_argument("--runs", type=int, default=16)
+    ap.add_argument("--cap", type=int, default=200000)
+    ap.add_argument("--chunk", type=int, default=100)
+    ap.add_argument("--seed0", type=int, default=100)
+    args = ap.parse_args()
+    rows = []
+    for n in args.n:
+        r = run_size(n, args.words, args.instances, args.runs, args.cap, args.chunk, args.seed0)
+        rows.append(r)
+        print(json.dumps(r), flush=True)
+    # exponential growth of the typical time with N (L151: TTS_99 ~ exp(a N), a = 0.0786(4))
+    pts = [(r["n_spins"], math.log(r["median_tau_sweeps"] * r["clones"])) for r in rows
+           if r["median_tau_sweeps"]]
+    if len(pts) >= 2:
+        xs_, ys_ = np.array([p[0] for p in pts], float), np.array([p[1] for p in pts], float)
+        a, c = np.polyfit(xs_, ys_, 1)
+        print(json.dumps({"fit": "ln(t0) = a N + c over solved sizes", "a": float(a), "c": float(c),
+                          "sizes": [p[0] for p in pts], "paper_a": 0.0786}), flush=True)
+
+
+if __name__ == "__main__":
+    main()

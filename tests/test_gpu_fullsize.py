@@ -1,0 +1,102 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (library
+defaults, no geometry overrides), on sampled words the oracle can follow one by one
+(SURVEY.md 8(c) protocol (ii): words evolve independently given (seed, w))."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from _harness import OracleRun  # noqa: E402
+from oracle.xs_oracle import NO_HIT  # noqa: E402
+
+
+@pytest.fixture(autouse=True)
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
+
+
+def _check_words(b, o, inst=0):
+    x = b.spins_numpy()[inst]
+    fh = b.first_hit_numpy()[inst]
+    e = b.energy().cpu().numpy()[inst]
+    xo, eo = o.x(), o.energy()
+    for w in o.words:
+        sl = slice(64 * w, 64 * w + 64)
+        assert np.array_equal(x[:, w], xo[:, w]), f"spin words differ in word {w}"
+        assert np.array_equal(fh[sl], o.first_hit[sl]), f"first hits differ in word {w}"
+        assert np.array_equal(e[sl], eo[sl]), f"energies differ in word {w}"
+
+
+def test_config2_full_size_sampled_words():
+    """configs[1]: N=256, graph seed 2, 2^16 clones; bench.py's geometry (static kernel, T=8)."""
+    import paper_2102_09510_b200 as xs
+    N, W = 256, 1024
+    b = xs.Batch(N, W, [2], [2], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
+    lay = b.layout()
+    assert (lay.regime, lay.variant, lay.tile_words, lay.ctas) == (0, 1, 8, 128)
+    words = [0, 7, 8, 517, 1023]          # first/last lane of a tile, tile boundaries, last tile
+    o = OracleRun(N, W, 2, 2, no_skip=True, words=words)
+    for n in (130, 171):                  # crosses batch boundaries (64) at odd offsets
+        b.run_sweeps(n)
+        o.run_sweeps(n)
+    _check_words(b, o)
+    # properties that hold for every clone at any size
+    e = b.energy().cpu().numpy()[0]
+    assert e.min() >= -N and (e % 2 == 0).all() and abs(e.mean() / N + 0.8957) < 0.02
+    r = b.tts()[0]
+    assert r.sweeps_done == 301 and r.solved == int((b.first_hit_numpy() != NO_HIT).any())
+    b.close()
+
+
+def test_config3_shape_sampled_instances_and_words():
+    """configs[2] shape: N=512, W=64 per instance, 160 instances so that every SM gets a tile
+    (generic kernel, T=16 -- the geometry the full 256-instance run uses)."""
+    import paper_2102_09510_b200 as xs
+    N, W, I = 512, 64, 160
+    seeds = list(range(100, 100 + I))
+    b = xs.Batch(N, W, seeds, seeds)
+    lay = b.layout()
+    assert (lay.regime, lay.variant, lay.tile_words) == (0, 0, 16)
+    checks = {0: [0, 15, 16], 77: [33, 63], 159: [48]}
+    oracles = {i: OracleRun(N, W, seeds[i], seeds[i], words=ws) for i, ws in checks.items()}
+    b.run_sweeps(70)
+    for i, o in oracles.items():
+        o.run_sweeps(70)
+        _check_words(b, o, inst=i)
+    recs = b.tts()
+    assert all(r.sweeps_done == 70 for r in recs)
+    b.close()
+
+
+def test_config5_streaming_large_instance_sampled_word():
+    """configs[4] regime at N = 2^16 (2^20 is exercised by bench.py --workload config5): state
+    does not fit on chip -> streaming kernel, W = 16 (128-byte rows)."""
+    import paper_2102_09510_b200 as xs
+    N, W = 1 << 16, 16
+    b = xs.Batch(N, W, [5], [5], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
+    assert b.layout().regime == 1
+    o = OracleRun(N, W, 5, 5, no_skip=True, words=[3])
+    b.run_sweeps(3)
+    o.run_sweeps(3)
+    _check_words(b, o)
+    e = b.energy().cpu().numpy()[0]
+    assert e.min() >= -N and (e % 2 == 0).all()
+    b.close()
+
+
+def test_max_tile_and_ragged_shapes():
+    """Edge shapes: N = 3 (smallest legal), N not a multiple of anything, W = 1, W = 24 (T = 8),
+    one 64-column tile."""
+    import paper_2102_09510_b200 as xs
+    for N, W, sweeps in [(3, 1, 5), (7, 2, 9), (131, 24, 11), (67, 64, 9), (37, 5, 12)]:
+        b = xs.Batch(N, W, [N], [2 * N], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
+        o = OracleRun(N, W, N, 2 * N, no_skip=True)
+        b.run_sweeps(sweeps)
+        o.run_sweeps(sweeps)
+        _check_words(b, o)
+        b.close()

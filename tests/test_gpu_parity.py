@@ -81,6 +81,7 @@ def test_init_state_and_energy():
     (64, 1, 300, 0),      # config-1 shape: one word, CW=1 path
     (96, 4, 120, 0),
     (96, 6, 60, 0),       # W not a power of two -> T = 2
+    (200, 4, 40, 4),      # T = 4: static kernel with four row copies (variant 1)
     (256, 8, 40, 8),      # config-2 tile shape (T = 8)
     (256, 16, 24, 16),
     (130, 32, 20, 32),
@@ -111,6 +112,7 @@ def test_sweep_parity_all_words(N, W, sweeps, tile, variant):
     (100, 16, 16, 512, 23),
     (60, 32, 32, 512, 21),
     (18, 8, 8, 128, 45),      # many solved clones: replay path with a 4-sweep noise period
+    (100, 4, 4, 128, 33),     # T = 4: four row copies per 128-byte line
 ])
 def test_static_kernel_one_word_per_lane(N, W, tile, threads, sweeps):
     """Static-task kernel with CW = 1: four lanes share a Philox call over a 4-sweep period."""
@@ -161,7 +163,7 @@ def test_first_hit_exact_many_solved_clones(batch, streaming, W):
     xs = _xs()
     N = 18
     flags = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_STREAMING if streaming else 0)
-    with env(XS_BATCH=batch):
+    with env(XS_BATCH=batch, XS_VARIANT=(1 if W == 8 else 0)):
         b = xs.Batch(N, W, [5], [9], flags=flags)
     assert b.layout().regime == (1 if streaming else 0)
     if not streaming:
