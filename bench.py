@@ -41,6 +41,10 @@ WORKLOADS = {
 }
 ALU_OPS_PER_UPDATE = 14.0 / 32.0      # 14 LOP3/IADD lane-ops per 32 clone-spin updates
 STREAM_BYTES_PER_UPDATE = (8 * 8 * 16 + 28) / 1024.0   # config 5, W=16: 1052 B per 1024 updates
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu
+# --set full captures summarised in profiles/r01_ncu_summary.md (config5: the launch of the
+# largest independent set, 262,053 spin rows = 275.7 MB algorithmic).
+NCU_DRAM_BYTES_PER_LAUNCH = {"config2": 2.43e6, "config3": 91.6e6, "config5": 187.9e6}
 
 
 class ClockSampler:
@@ -93,7 +97,7 @@ def cpu_oracle_rate(wl, target_s: float = 12.0):
     cores = omp_threads()
     N = wl["N"]
     inst = Instance(N, wl["graph_seed"], True, 0)
-    W = max(1, min(wl["W"], cores))
+    W = max(1, min(wl["W"], 4 * cores))      # enough words for ~target_s of work on all cores
     s = inst.init_spins(W, wl["run_seed"])
     fh = np.full(64 * W, NO_HIT, np.uint32)
     t0 = time.perf_counter()
@@ -258,15 +262,15 @@ def main():
         if lay.regime == 0:
             achieved = ALU_OPS_PER_UPDATE * updates_per_step / (k_ms * 1e6) / 1e3      # Tlop/s
             roof = {"bound": "alu", "achieved": achieved, "peak": alu_peak / 1e3, "unit": "Tlop/s (32-bit LOP3/IADD lane-ops)",
-                    "frac": achieved / (alu_peak / 1e3), "traffic": None,
+                    "frac": achieved / (alu_peak / 1e3), "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload),
                     "peak_source": "xs_alu_peak LOP3 micro-kernel measured in this run",
                     "peak_nominal_at_sampled_clock": (148 * 64 * clocks["sm_mhz"] / 1e6) if clocks.get("sm_mhz") else None,
-                    "alg_ops_per_update": ALU_OPS_PER_UPDATE, "kernel": "k_sweep_tile", "kernel_ms": k_ms}
+                    "alg_ops_per_update": ALU_OPS_PER_UPDATE, "kernel": "k_sweep_static" if lay.variant == 1 else "k_sweep_tile", "kernel_ms": k_ms}
         else:
             hbm = peaks.get("hbm_gbs", 6650.0)
             achieved = STREAM_BYTES_PER_UPDATE * updates_per_step / (k_ms * 1e6)          # GB/s
             roof = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
-                    "traffic": None, "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "fallback 6650 GB/s",
+                    "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "fallback 6650 GB/s",
                     "alg_bytes_per_update": STREAM_BYTES_PER_UPDATE, "kernel": "k_stream_set", "kernel_ms": k_ms}
         e_np = e_last.cpu().numpy()
         out = {

@@ -680,6 +680,18 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     g.ctas = p.n_instances * (p.n_words / g.T);
     uint32_t rb = std::min(g.batch, env_u32("XS_RB", 8));
     while (rb > 1 && tile_smem(p.n_spins, g.T, rb, b.n_sets_max).total > SMEM_MAX) --rb;
+    // Two CTAs per SM overlap each other's load / compute / barrier phases (measured +19 % on
+    // config 3, profiles/r01_ncu_summary.md): shrink the noise ring and the CTA until two fit
+    // (228 KB shared memory and 64 K registers per SM; this kernel uses 56 registers).
+    if (!env_u32("XS_RB", 0) && g.ctas >= 2 * NUM_SMS) {
+        const uint32_t sm_smem = 228u * 1024u, reserved = 1024u;
+        uint32_t r2 = rb;
+        while (r2 > 1 && 2 * (tile_smem(p.n_spins, g.T, r2, b.n_sets_max).total + reserved) > sm_smem) r2 /= 2;
+        if (2 * (tile_smem(p.n_spins, g.T, r2, b.n_sets_max).total + reserved) <= sm_smem) {
+            rb = r2;
+            if (!env_u32("XS_THREADS", 0)) g.threads = std::min(g.threads, 512u);
+        }
+    }
     g.rb = rb;
     g.smem = tile_smem(p.n_spins, g.T, rb, b.n_sets_max).total;
     return true;
