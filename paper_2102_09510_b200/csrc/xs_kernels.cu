@@ -593,7 +593,7 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     const uint32_t force_T = env_u32("XS_TILE_WORDS", 0);
     uint32_t bestT = 0;
     uint64_t best_cost = ~0ull;
-    // Measured on B200 (profiles/geometry_sweep_r01.md): with at least one 16-column tile per SM
+    // Measured on B200: with at least one 16-column tile per SM
     // the generic kernel with T = 16 (128-byte rows: conflict-free, several CTAs per SM overlap
     // their load / compute / barrier phases) is the fastest choice; with fewer tiles than SMs
     // (config 2) the static-task kernel with T = 8 wins because one CTA per SM must hide its

@@ -1,0 +1,54 @@
+"""The Boolean form the kernels use (csrc/xs_device.cuh, a-4..a-7) against the +-1 rule of the
+paper, exhaustively over all 2^11 inputs: 6 partner bits, 3 coupling
+bits, own bit, noise bit.  The LOP3 truth-table constants are read from the CUDA header, so a
+wrong LUT in the product fails here without a GPU."""
+from __future__ import annotations
+
+import itertools
+import os
+import re
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _luts():
+    src = open(os.path.join(ROOT, "paper_2102_09510_b200", "csrc", "xs_device.cuh")).read()
+    out = {}
+    for name in ("LUT_XOR3", "LUT_MAJ", "LUT_MAJ_NOTC", "LUT_SEL", "LUT_NZ"):
+        m = re.search(r"constexpr int %s = (0x[0-9A-Fa-f]+);" % name, src)
+        assert m, name
+        out[name] = int(m.group(1), 16)
+    # the order of the lop3 calls in qg_update / qg_nonzero_k is part of what is checked
+    assert re.search(r"w0 = lop3<LUT_XOR3>\(a0, b0, j0\)", src)
+    assert re.search(r"M = lop3<LUT_MAJ>\(w0, w1, w2\)", src)
+    assert re.search(r"P = lop3<LUT_XOR3>\(w0, w1, w2\)", src)
+    assert re.search(r"f = lop3<LUT_MAJ_NOTC>\(M, P, x\)", src)
+    assert re.search(r"return lop3<LUT_SEL>\(R, f, M\)", src)
+    assert re.search(r"return lop3<LUT_NZ>\(M, P, x\)", src)
+    return out
+
+
+def lop3(lut, a, b, c):
+    return (lut >> (a * 4 + b * 2 + c)) & 1      # PTX lop3: bit index = a*4 + b*2 + c
+
+
+def test_boolean_update_equals_pm1_rule_on_all_inputs():
+    L = _luts()
+    for bits in itertools.product((0, 1), repeat=11):
+        a0, b0, a1, b1, a2, b2, j0, j1, j2, x, R = bits
+        # +-1 arithmetic: bit 1 <=> spin -1, jbit 1 <=> J = -1
+        s = lambda v: 1 - 2 * v                                    # noqa: E731
+        k = sum(1 for (a, b, j) in ((a0, b0, j0), (a1, b1, j1), (a2, b2, j2))
+                if s(j) * s(x) * s(a) * s(b) == -1)                # unsatisfied interactions
+        flip = (k >= 2) or (k == 1 and R == 1)                     # w = (0, w1, 1, 1)
+        x_new_ref = x ^ int(flip)
+        # Boolean form
+        w0, w1, w2 = (lop3(L["LUT_XOR3"], a0, b0, j0), lop3(L["LUT_XOR3"], a1, b1, j1),
+                      lop3(L["LUT_XOR3"], a2, b2, j2))
+        M, P = lop3(L["LUT_MAJ"], w0, w1, w2), lop3(L["LUT_XOR3"], w0, w1, w2)
+        f = lop3(L["LUT_MAJ_NOTC"], M, P, x)
+        x_new = lop3(L["LUT_SEL"], R, f, M)
+        assert x_new == x_new_ref, bits
+        assert lop3(L["LUT_NZ"], M, P, x) == int(k != 0), bits
+        assert 2 * (M ^ x) + (P ^ x) == k, bits                    # the bit-sliced adder
+        assert 6 - 4 * k in (6, 2, -2, -6)                         # Delta E of the flip (L67)
