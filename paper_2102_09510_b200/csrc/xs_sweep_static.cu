@@ -15,11 +15,12 @@
 // exactly once and nothing goes through shared memory.
 //
 // Bank conflicts: for T = 8 a spin row is 64 B, so the two spins served by one 128-byte phase
-// of a shared load collide when their rows have the same parity.  DUP keeps two copies of
-// every row in one 128 B line (banks 0-15 and 16-31); even slots read copy 0, odd slots copy
-// 1, and a write updates both copies in two conflict-free stores.  T >= 16 rows are whole
-// 128 B lines and need no copy.  Lanes without a task in a round work on a scratch line, so
-// the hot loop has no per-lane branch.
+// of a shared load collide when their rows have the same parity.  The kernel keeps NC = 16 / T
+// copies of every row in one 128 B line (T = 8: banks 0-15 and 16-31; T = 4: four quarters);
+// slot s reads copy s % NC, and a write updates all copies in NC conflict-free stores (in
+// store c, slot s writes copy (s + c) % NC).  T >= 16 rows are whole 128 B lines and need no
+// copy.  Lanes without a task in a round work on a scratch line, so the hot loop has no
+// per-lane branch; warps without any task skip the round.
 //
 // Ground-state detection / exact first hit: as in k_sweep_tile (detection pass every `batch`
 // sweeps, replay of the batch from the global copy with a pass after every sweep, L293).
@@ -39,7 +40,6 @@ struct StaticArgs {
     uint32_t N, W, T, n_sweeps, thr, flags, batch;
     uint32_t line_shift;   // log2(bytes of one spin line in shared memory)
     uint32_t off_misc;     // byte offset of det32 / known32 / flag in dynamic shared memory
-    uint32_t dbg;          // timing ablations (XS_DBG, wrong results): 1 no barriers, 2 no noise, 4 one store, 8 no loads
 };
 
 // CW uint64 words = 2*CW uint32 per lane, by 32-bit shared address
@@ -248,7 +248,7 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
 #pragma unroll
                     for (int c = 0; c < H; ++c) tk.x[r][c] = xn[c];
                 }
-                if (((tk.bar >> r) & 1u) && !(A.dbg & 1u)) __syncthreads();
+                if ((tk.bar >> r) & 1u) __syncthreads();
             }
         }
     };
@@ -289,13 +289,12 @@ __global__ void __launch_bounds__(MAXTHREADS, 1) k_sweep_static(StaticArgs A)
             if (have_next) {
 #pragma unroll
                 for (int r = 0; r < MAXT; ++r) tk.rm[r] = tk.rmn[r];
-            } else if (!(A.dbg & 2u)) {
+            } else {
                 produce_all(q);
             }
             // the next period's noise can be produced inside this period's sweeps iff all NL
             // sweeps of this period run and there is a next period
-            const bool fuse = (NL * q >= t_first) && (NL * q + NL - 1 <= t_last) && (q < q_last) &&
-                              !(A.dbg & 2u);
+            const bool fuse = (NL * q >= t_first) && (NL * q + NL - 1 <= t_last) && (q < q_last);
             auto step = [&](auto hc) {
                 const uint32_t t = NL * q + decltype(hc)::value;
                 if (t < t_first || t > t_last) return;
@@ -403,13 +402,12 @@ static cudaError_t launch_k(const StaticArgs& A, uint32_t ctas, uint32_t threads
     k_sweep_static<MAXT, CW, NC, MT><<<ctas, threads, smem, st>>>(A);
     return cudaGetLastError();
 }
-static uint32_t g_rounds_for_launch = STATIC_MAXT;
 template <int CW, int NC, int MT>
 static cudaError_t launch_one(const StaticArgs& A, uint32_t ctas, uint32_t threads, uint32_t smem,
-                              cudaStream_t st)
+                              cudaStream_t st, uint32_t rounds)
 {
     // fewer unrolled rounds = fewer registers (the 512-thread variants are capped at 128)
-    if (g_rounds_for_launch <= 6) return launch_k<6, CW, NC, MT>(A, ctas, threads, smem, st);
+    if (rounds <= 6) return launch_k<6, CW, NC, MT>(A, ctas, threads, smem, st);
     return launch_k<STATIC_MAXT, CW, NC, MT>(A, ctas, threads, smem, st);
 }
 
@@ -423,15 +421,14 @@ int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream)
     A.thr = p.w1_threshold; A.flags = p.flags; A.batch = g.batch;
     A.line_shift = static_line_shift(g.T);
     A.off_misc = (uint32_t)((((uint64_t)p.n_spins + 1) << A.line_shift) + 127) / 128 * 128;
-    { const char* s_ = std::getenv("XS_DBG"); A.dbg = s_ ? (uint32_t)std::atoi(s_) : 0u; }
     cudaStream_t st = (cudaStream_t)stream;
     const uint32_t nc = g.T <= 16 ? 16u / g.T : 1u;     // row copies per 128-byte line
     const bool small = g.threads <= 256;
-    g_rounds_for_launch = static_rounds(b, g.T, g.CW, g.threads);
+    const uint32_t rounds = static_rounds(b, g.T, g.CW, g.threads);
     cudaError_t e;
 #define XS_STATIC_LAUNCH(CWV, NCV)                                                          \
-    e = small ? launch_one<CWV, NCV, 256>(A, g.ctas, g.threads, g.smem, st)                 \
-              : launch_one<CWV, NCV, 512>(A, g.ctas, g.threads, g.smem, st)
+    e = small ? launch_one<CWV, NCV, 256>(A, g.ctas, g.threads, g.smem, st, rounds)         \
+              : launch_one<CWV, NCV, 512>(A, g.ctas, g.threads, g.smem, st, rounds)
     if (g.CW == 2) {
         if (nc == 4) XS_STATIC_LAUNCH(2, 4); else if (nc == 2) XS_STATIC_LAUNCH(2, 2); else XS_STATIC_LAUNCH(2, 1);
     } else {

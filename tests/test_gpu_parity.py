@@ -189,13 +189,16 @@ def test_streaming_regime_matches_oracle():
         b.close()
 
 
-def test_multi_instance_stop_rule():
+@pytest.mark.parametrize("streaming", [False, True])
+def test_multi_instance_stop_rule(streaming):
     """Instances that have a solved clone at call entry are skipped (L129/L293 stop rule)."""
     xs = _xs()
     N, W = 32, 1
     gseeds = list(range(3, 11))
     rseeds = list(range(13, 21))
-    b = xs.Batch(N, W, gseeds, rseeds)
+    b = xs.Batch(N, W, gseeds, rseeds,
+                 flags=xs.XS_FLAG_GAUGE | (xs.XS_FLAG_STREAMING if streaming else 0))
+    assert b.layout().regime == int(streaming)
     os_ = [OracleRun(N, W, g, r) for g, r in zip(gseeds, rseeds)]
     for _ in range(10):
         b.run_sweeps(20)
