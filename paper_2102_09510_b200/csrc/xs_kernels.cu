@@ -605,7 +605,10 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     uint32_t auto_T = 0;
     if (want_variant == 2 && many_tiles && !force_T) auto_T = 16;
     // 1) static-task kernel (xs_sweep_static.cu): work list in registers, T in {8,16,32,64}
-    if (!(p.flags & XS_FLAG_STREAMING) && (want_variant == 1 || (want_variant == 2 && !auto_T))) {
+    // many small tiles (e.g. 20,000 runs of W = 4): the generic kernel's high occupancy wins
+    const bool few_tiles = (uint64_t)p.n_instances * ((p.n_words + 7) / 8) < 2ull * NUM_SMS;
+    if (!(p.flags & XS_FLAG_STREAMING) &&
+        (want_variant == 1 || (want_variant == 2 && !auto_T && few_tiles))) {
         const uint32_t force_thr = env_u32("XS_THREADS", 0);
         const uint32_t force_cw = env_u32("XS_CW", 0);
         uint32_t sT = 0, sThr = 0, sCW = 0;
@@ -643,18 +646,24 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     }
     // 2) generic tile kernel
     if (!(p.flags & XS_FLAG_STREAMING) && (uint64_t)p.n_spins * 8 < SMEM_MAX) {
-        for (uint32_t T = 64; T >= 1; T >>= 1) {
-            if (p.n_words % T) continue;
-            if (force_T && T != force_T) continue;
-            if (auto_T && T != auto_T) continue;
-            const TileSmem s = tile_smem(p.n_spins, T, 1, b.n_sets_max);
-            if (s.total > SMEM_MAX) continue;
-            const uint64_t ctas = (uint64_t)p.n_instances * (p.n_words / T);
-            const uint32_t occ = std::max(1u, std::min(SMEM_MAX / s.total, 2048u / 1024u));
-            const uint64_t waves = (ctas + (uint64_t)NUM_SMS * occ - 1) / ((uint64_t)NUM_SMS * occ);
-            const uint64_t cost = waves * T * occ;
-            if (cost < best_cost) { best_cost = cost; bestT = T; }
+        // Widest tile (up to a 128-byte row) that still gives every SM two CTAs, else one CTA,
+        // else the narrowest tile (most CTAs).  Wider tiles share records and Philox calls
+        // between more clone words; narrow rows cost bank conflicts.
+        auto ok = [&](uint32_t T) {
+            if (p.n_words % T) return false;
+            if (force_T && T != force_T) return false;
+            if (auto_T && T != auto_T) return false;
+            return tile_smem(p.n_spins, T, 1, b.n_sets_max).total <= SMEM_MAX;
+        };
+        auto n_ctas = [&](uint32_t T) { return (uint64_t)p.n_instances * (p.n_words / T); };
+        for (uint64_t want : {2ull * NUM_SMS, 1ull * NUM_SMS}) {
+            for (uint32_t T = 16; T >= 1 && !bestT; T >>= 1)
+                if (ok(T) && n_ctas(T) >= want) bestT = T;
+            if (bestT) break;
         }
+        for (uint32_t T = 1; T <= 64 && !bestT; T <<= 1)
+            if (ok(T)) bestT = T;
+        (void)best_cost;
     }
     if (bestT == 0) {
         g.regime = 1;

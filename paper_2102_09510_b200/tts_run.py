@@ -54,6 +54,28 @@ def run_size(n, words, instances, runs, cap, chunk, seed0, flags_extra=0):
     taus = np.array([s["tau_hat"] for s in per_inst])
     tts99 = np.array([s["tts99_model"] for s in per_inst])
     n_solved_runs = int((tts != xs.XS_NO_HIT).sum())
+    # PAPER.md Eq. (2), Fig. 2: P[TTS > t] = exp(-t / tau).  Per instance with all runs solved:
+    # Kolmogorov-Smirnov distance between the empirical distribution of the R TTS values and
+    # 1 - exp(-t / tau_hat), and the empirical / model ratios of TTS_50 and TTS_99 (Fig. 3).
+    ks, r50, r99, ks_shift, t_min_over_tau = [], [], [], [], []
+    for i in range(instances):
+        if per_inst[i]["n_solved"] < runs or runs < 8:
+            continue
+        v = np.sort(tts[i].astype(np.float64))
+        cdf = 1.0 - np.exp(-v / per_inst[i]["tau_hat"])
+        k = np.arange(1, runs + 1) / runs
+        ks.append(float(max(np.max(k - cdf), np.max(cdf - (k - 1.0 / runs)))))
+        # same with an onset time: no clone can hit before the initial relaxation, so at finite
+        # tau the law is exp(-(t - t_on) / (tau - t_on)); t_on estimated by the smallest TTS
+        t_on = v[0] - (v.mean() - v[0]) / runs
+        cdf_s = 1.0 - np.exp(-np.maximum(v - t_on, 0.0) / (v.mean() - t_on))
+        ks_shift.append(float(max(np.max(k - cdf_s), np.max(cdf_s - (k - 1.0 / runs)))))
+        t_min_over_tau.append(float(t_on / v.mean()))
+        r50.append(per_inst[i]["tts50_emp"] / per_inst[i]["tts50_model"])
+        r99.append(per_inst[i]["tts99_emp"] / per_inst[i]["tts99_model"])
+    # KS critical value at 1 % for a fully specified law is 1.63 / sqrt(R); with tau estimated
+    # from the same data (Lilliefors, exponential) it is about 1.25 / sqrt(R)
+    ks_crit = 1.25 / math.sqrt(runs) if runs else None
     solved_inst = int(sum(1 for s in per_inst if s["n_solved"] > 0))
     med = lambda a: float(np.median(a)) if np.isfinite(np.median(a)) else None   # noqa: E731
     lower = [s["tau_q16"] for s in per_inst if s["n_solved"] == 0]
@@ -72,6 +94,15 @@ def run_size(n, words, instances, runs, cap, chunk, seed0, flags_extra=0):
         "sec_per_sweep_per_run": sec_per_sweep,
         "median_tts99_seconds": (med(tts99) * sec_per_sweep) if med(tts99) else None,
         "updates_per_ns": n * clones * unsolved_sweeps / max(gpu_ms * 1e6, 1e-9),
+        "survival_ks_median": float(np.median(ks)) if ks else None,
+        "survival_ks_max": float(np.max(ks)) if ks else None,
+        "survival_ks_crit_1pct": ks_crit,
+        "survival_ks_fraction_below_crit": float(np.mean(np.array(ks) < ks_crit)) if ks else None,
+        "survival_ks_with_onset_median": float(np.median(ks_shift)) if ks_shift else None,
+        "survival_ks_with_onset_fraction_below_crit": float(np.mean(np.array(ks_shift) < ks_crit)) if ks_shift else None,
+        "onset_over_tau_median": float(np.median(t_min_over_tau)) if t_min_over_tau else None,
+        "tts50_emp_over_model_median": float(np.median(r50)) if r50 else None,
+        "tts99_emp_over_model_median": float(np.median(r99)) if r99 else None,
         "gpu_ms": gpu_ms, "wall_s": time.time() - t0,
     }
     b.close()
