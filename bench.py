@@ -38,7 +38,14 @@ WORKLOADS = {
                     desc="configs[4]: N=2^20, 1 instance (graph seed 5), 2^10 clones, 100 sweeps (streaming)"),
     "config3": dict(N=512, W=64, I=256, sweeps=2_000, graph_seed=100, run_seed=100,
                     desc="configs[2] shape: N=512, 256 instances (seeds 100..355), 2^12 clones each, 2000 sweeps per step"),
+    # SURVEY.md F3 / 8(d) "5b": as config 5 with 2^14 clones = 2 GiB of state, DRAM resident
+    "config5b": dict(N=1 << 20, W=256, I=1, sweeps=10, graph_seed=5, run_seed=5,
+                     desc="config 5b: N=2^20, 1 instance (graph seed 5), 2^14 clones (2 GiB state), 10 sweeps (streaming)"),
 }
+# configs[3] shapes: 128 instances (graph seeds 1000 N + i), 2^14 clones each
+for _n, _s in ((128, 2000), (192, 1500), (256, 1000), (384, 700), (512, 500), (768, 350), (1024, 250)):
+    WORKLOADS[f"config4_{_n}"] = dict(N=_n, W=256, I=128, sweeps=_s, graph_seed=1000 * _n, run_seed=1000 * _n,
+                                      desc=f"configs[3] shape: N={_n}, 128 instances, 2^14 clones each, {_s} sweeps per step")
 ALU_OPS_PER_UPDATE = 14.0 / 32.0      # 14 LOP3/IADD lane-ops per 32 clone-spin updates
 STREAM_BYTES_PER_UPDATE = (8 * 8 * 16 + 28) / 1024.0   # config 5, W=16: 1052 B per 1024 updates
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu
@@ -268,10 +275,11 @@ def main():
                     "alg_ops_per_update": ALU_OPS_PER_UPDATE, "kernel": "k_sweep_static" if lay.variant == 1 else "k_sweep_tile", "kernel_ms": k_ms}
         else:
             hbm = peaks.get("hbm_gbs", 6650.0)
-            achieved = STREAM_BYTES_PER_UPDATE * updates_per_step / (k_ms * 1e6)          # GB/s
+            bpu = (8 * 8 * W + 28) / (64.0 * W)      # 6 partner rows + own row read + write + record
+            achieved = bpu * updates_per_step / (k_ms * 1e6)                              # GB/s
             roof = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "fallback 6650 GB/s",
-                    "alg_bytes_per_update": STREAM_BYTES_PER_UPDATE, "kernel": "k_stream_set", "kernel_ms": k_ms}
+                    "alg_bytes_per_update": bpu, "kernel": "k_stream_set", "kernel_ms": k_ms}
         e_np = e_last.cpu().numpy()
         out = {
             "metric": "clone-spin updates/ns", "value": value, "unit": "clone-spin updates/ns", "n_gpus": world,

@@ -46,6 +46,33 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
 }
 
+// Same with the 10 round keys precomputed (the key is fixed per instance: keeps the key
+// schedule's 20 additions out of every call).
+__device__ __forceinline__ void philox_key_schedule(uint32_t k0, uint32_t k1, uint32_t (&ks)[10][2])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        ks[r][0] = k0 + (uint32_t)r * 0x9E3779B9u;
+        ks[r][1] = k1 + (uint32_t)r * 0xBB67AE85u;
+    }
+}
+__device__ __forceinline__ void philox4x32_10_ks(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                 const uint32_t (&ks)[10][2], uint32_t o[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0);
+        const uint32_t l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2);
+        const uint32_t l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ ks[r][0];
+        c2 = h0 ^ c3 ^ ks[r][1];
+        c1 = l1;
+        c3 = l0;
+    }
+    o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
+}
+
 // One QG update of 32 clones.  a*/b* partner words, j* coupling masks, x own word, R noise mask.
 __device__ __forceinline__ uint32_t qg_update(uint32_t a0, uint32_t b0, uint32_t j0, uint32_t a1,
                                               uint32_t b1, uint32_t j1, uint32_t a2, uint32_t b2,

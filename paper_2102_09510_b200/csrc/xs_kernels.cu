@@ -285,29 +285,33 @@ __device__ __forceinline__ void tile_detect_acc(const TileCtx<CW>& c)
         if (acc[h]) atomicOr(&c.det32[2 * c.jw + h], acc[h]);
 }
 
-// Noise bytes for sweeps t_first .. t_first + ns - 1 (a-6).
+// Noise bytes for sweeps t_first .. t_first + ns - 1 (a-6).  One Philox call per (sweep,
+// position, group of 4 words); round keys precomputed; G is a power of two (no divisions).
 template <int CW>
 __device__ __forceinline__ void tile_produce(const TileCtx<CW>& c, uint32_t t_first, uint32_t ns,
-                                             uint32_t w0, uint32_t k0, uint32_t k1, uint32_t thr)
+                                             uint32_t w0, const uint32_t (&ks)[10][2], uint32_t thr)
 {
     const uint32_t G = c.T >= 4 ? c.T / 4 : 1;
-    const uint32_t per_sweep = c.N * G;
-    const uint32_t total = ns * per_sweep;
-    for (uint32_t e = threadIdx.x; e < total; e += blockDim.x) {
-        const uint32_t s = e / per_sweep;
-        const uint32_t q = e - s * per_sweep;
-        const uint32_t p = q / G, g = q - p * G;
-        const uint32_t spin = c.rec[3 * p + 1].w;
-        uint32_t o[4];
-        philox4x32_10(spin, (w0 >> 2) + g, t_first + s, TAG_SWEEP, k0, k1, o);
-        unsigned char* dst = c.rbuf + ((size_t)s * c.N + p) * c.T;
-        if (c.T >= 4) {
-            const uint32_t v = (o[0] < thr ? 0xFFu : 0u) | (o[1] < thr ? 0xFF00u : 0u) |
-                               (o[2] < thr ? 0xFF0000u : 0u) | (o[3] < thr ? 0xFF000000u : 0u);
-            *reinterpret_cast<uint32_t*>(dst + 4 * g) = v;
-        } else {
-            for (uint32_t lw = 0; lw < c.T; ++lw)
-                dst[lw] = o[(w0 + lw) & 3u] < thr ? 0xFF : 0;
+    const uint32_t gsh = (uint32_t)__ffs((int)G) - 1u;
+    const uint32_t per_sweep = c.N << gsh;
+    const uint32_t grp0 = w0 >> 2;
+    for (uint32_t s = 0; s < ns; ++s) {
+        unsigned char* row = c.rbuf + (size_t)s * c.N * c.T;
+        const uint32_t t = t_first + s;
+        for (uint32_t q = threadIdx.x; q < per_sweep; q += blockDim.x) {
+            const uint32_t p = q >> gsh, g = q & (G - 1u);
+            const uint32_t spin = c.rec[3 * p + 1].w;
+            uint32_t o[4];
+            philox4x32_10_ks(spin, grp0 + g, t, TAG_SWEEP, ks, o);
+            unsigned char* dst = row + (size_t)p * c.T;
+            if (c.T >= 4) {
+                const uint32_t v = (o[0] < thr ? 0xFFu : 0u) | (o[1] < thr ? 0xFF00u : 0u) |
+                                   (o[2] < thr ? 0xFF0000u : 0u) | (o[3] < thr ? 0xFF000000u : 0u);
+                *reinterpret_cast<uint32_t*>(dst + 4 * g) = v;
+            } else {
+                for (uint32_t lw = 0; lw < c.T; ++lw)
+                    dst[lw] = o[(w0 + lw) & 3u] < thr ? 0xFF : 0;
+            }
         }
     }
 }
@@ -343,6 +347,8 @@ __global__ void __launch_bounds__(1024, 1) k_sweep_tile(TileArgs A)
 
     const uint64_t seed = A.d.run_seed[inst];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    uint32_t ks[10][2];
+    philox_key_schedule(k0, k1, ks);
     uint64_t* xg = A.d.x + (size_t)inst * N * W + w0;
     uint32_t* fhg = A.d.first_hit + ((size_t)inst * W + w0) * 64;
     const uint32_t row_bytes = T * 8;
@@ -393,7 +399,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep_tile(TileArgs A)
     auto run_range = [&](uint32_t t0, uint32_t n, bool exact) {
         for (uint32_t s0 = 0; s0 < n; s0 += A.rb) {
             const uint32_t ns = min(A.rb, n - s0);
-            tile_produce<CW>(c, t0 + s0 + 1, ns, w0, k0, k1, A.thr);
+            tile_produce<CW>(c, t0 + s0 + 1, ns, w0, ks, A.thr);
             __syncthreads();
             for (uint32_t s = 0; s < ns; ++s) {
                 tile_sweep<CW>(c, s);
