@@ -208,14 +208,14 @@ struct TileArgs {
 template <int CW>
 struct TileCtx {
     unsigned char* state;     // [N][T] uint64
-    const uint4* rec;         // [N][3]
+    const uint4* rec;         // [N][2]: {o0,o1,o2,o3}, {o4,o5,own offset, coupling bytes}
     unsigned char* rbuf;      // [rb][N][T] bytes
     const uint32_t* sets;     // [n_sets + 1]
     uint32_t* det32;          // [2T]
     uint32_t* known32;        // [2T]
     uint32_t* flag;
     uint32_t N, T, n_sets, slot, n_slots, joff /* byte offset of this lane's words in a row */,
-        jw /* first local word of this lane */;
+        jw /* first local word of this lane */, row_shift /* log2(bytes of a row) */;
 };
 
 template <int CW>
@@ -223,7 +223,7 @@ __device__ __forceinline__ void tile_gather(const TileCtx<CW>& c, uint32_t p, ui
                                             uint32_t (&b)[3][2 * CW], uint32_t (&x)[2 * CW],
                                             uint32_t (&jm)[3], uint32_t& self_off)
 {
-    const uint4 r0 = c.rec[3 * p], r1 = c.rec[3 * p + 1], r2 = c.rec[3 * p + 2];
+    const uint4 r0 = c.rec[2 * p], r1 = c.rec[2 * p + 1];
     vload<CW>(c.state + r0.x + c.joff, a[0]);
     vload<CW>(c.state + r0.y + c.joff, b[0]);
     vload<CW>(c.state + r0.z + c.joff, a[1]);
@@ -232,7 +232,10 @@ __device__ __forceinline__ void tile_gather(const TileCtx<CW>& c, uint32_t p, ui
     vload<CW>(c.state + r1.y + c.joff, b[2]);
     vload<CW>(c.state + r1.z + c.joff, x);
     self_off = r1.z;
-    jm[0] = r2.x; jm[1] = r2.y; jm[2] = r2.z;
+    // coupling masks from the bytes 0x00 / 0xFF of r1.w (sign extension = one PRMT each)
+    jm[0] = (uint32_t)(int32_t)(int8_t)(r1.w & 0xFFu);
+    jm[1] = (uint32_t)(int32_t)(int8_t)((r1.w >> 8) & 0xFFu);
+    jm[2] = (uint32_t)(int32_t)(int8_t)((r1.w >> 16) & 0xFFu);
 }
 
 // one sweep over all sets, sweep slot `rs` of the random-byte ring
@@ -300,7 +303,7 @@ __device__ __forceinline__ void tile_produce(const TileCtx<CW>& c, uint32_t t_fi
         const uint32_t t = t_first + s;
         for (uint32_t q = threadIdx.x; q < per_sweep; q += blockDim.x) {
             const uint32_t p = q >> gsh, g = q & (G - 1u);
-            const uint32_t spin = c.rec[3 * p + 1].w;
+            const uint32_t spin = c.rec[2 * p + 1].z >> c.row_shift;
             uint32_t o[4];
             philox4x32_10_ks(spin, grp0 + g, t, TAG_SWEEP, ks, o);
             unsigned char* dst = row + (size_t)p * c.T;
@@ -338,6 +341,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep_tile(TileArgs A)
     c.known32 = c.det32 + 2 * T;
     c.flag = c.known32 + 2 * T;
     c.N = N; c.T = T;
+    c.row_shift = 2u + (uint32_t)__ffs((int)T);      // T is a power of two: log2(8 T)
     c.n_sets = A.d.n_sets[inst];
     const uint32_t LPS = T / CW;
     c.slot = threadIdx.x / LPS;
@@ -357,12 +361,11 @@ __global__ void __launch_bounds__(1024, 1) k_sweep_tile(TileArgs A)
     const AdjRec* adj = A.d.adj + (size_t)inst * N;
     for (uint32_t p = threadIdx.x; p < N; p += blockDim.x) {
         const AdjRec r = adj[p];
-        rec_w[3 * p] = make_uint4(r.nbr[0] * row_bytes, r.nbr[1] * row_bytes, r.nbr[2] * row_bytes,
+        rec_w[2 * p] = make_uint4(r.nbr[0] * row_bytes, r.nbr[1] * row_bytes, r.nbr[2] * row_bytes,
                                   r.nbr[3] * row_bytes);
-        rec_w[3 * p + 1] = make_uint4(r.nbr[4] * row_bytes, r.nbr[5] * row_bytes, r.self * row_bytes,
-                                      r.self);
-        rec_w[3 * p + 2] = make_uint4((r.jbits & 1u) ? ~0u : 0u, (r.jbits & 2u) ? ~0u : 0u,
-                                      (r.jbits & 4u) ? ~0u : 0u, 0u);
+        rec_w[2 * p + 1] = make_uint4(r.nbr[4] * row_bytes, r.nbr[5] * row_bytes, r.self * row_bytes,
+                                      ((r.jbits & 1u) ? 0xFFu : 0u) | ((r.jbits & 2u) ? 0xFF00u : 0u) |
+                                          ((r.jbits & 4u) ? 0xFF0000u : 0u));
     }
     for (uint32_t s = threadIdx.x; s <= c.n_sets; s += blockDim.x)
         sets_w[s] = A.d.set_start[(size_t)inst * (N + 1) + s];
@@ -582,7 +585,7 @@ TileSmem tile_smem(uint32_t N, uint32_t T, uint32_t rb, uint32_t n_sets_max)
 {
     TileSmem s;
     uint64_t o = ((uint64_t)N * T * 8 + 15) / 16 * 16;   // records are read as 16-byte vectors
-    s.off_rec = (uint32_t)o;           o += (uint64_t)N * 48;
+    s.off_rec = (uint32_t)o;           o += (uint64_t)N * 32;
     s.off_rbuf = (uint32_t)o;          o += round_up(rb * N * T, 16);
     s.off_sets = (uint32_t)o;          o += round_up((n_sets_max + 1) * 4, 16);
     s.off_misc = (uint32_t)o;          o += round_up((4 * T + 4) * 4, 16);
