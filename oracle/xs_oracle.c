@@ -269,11 +269,15 @@ static int unsat_count(uint32_t i, const uint32_t* nbr, const uint32_t* cls,
  * n_flips (optional) counts accepted flips; dE_mismatch (optional) counts flips whose
  * incremental Delta E = 6 - 4k differs from E_after - E_before by full recomputation
  * (only evaluated when check_dE != 0; very slow). */
-void xso_sweep(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri,
-               const uint8_t* jbit, const uint32_t* nbr, const uint32_t* cls,
-               const uint32_t* order, const uint32_t* set_size, uint32_t n_sets,
-               uint64_t run_seed, uint32_t t, uint32_t w1_threshold, int mode,
-               int check_dE, int8_t* s, uint64_t* n_flips, uint64_t* dE_mismatch)
+/* General flip table (L67: "w_k the probability of flipping a spin entering k unsatisfied
+ * interactions"; L69: w0 = w1^3 with w2 = w3 = 1 satisfies detailed balance = Metropolis): thr4[k] in [0, 2^32], the spin
+ * flips iff u < thr4[k], with the SAME number u for every k (one number per word, L87).
+ * The quasi-greedy rule of L67/L101 is thr4 = (0, floor(0.055 2^32), 2^32, 2^32). */
+void xso_sweep_w(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri,
+                 const uint8_t* jbit, const uint32_t* nbr, const uint32_t* cls,
+                 const uint32_t* order, const uint32_t* set_size, uint32_t n_sets,
+                 uint64_t run_seed, uint32_t t, const uint64_t* thr4, int mode,
+                 int check_dE, int8_t* s, uint64_t* n_flips, uint64_t* dE_mismatch)
 {
     int8_t* snap = NULL;
     if (mode == 1) snap = (int8_t*)malloc(N);
@@ -287,9 +291,9 @@ void xso_sweep(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri
                     uint32_t i = order[p];
                     uint32_t o[4];
                     philox_seeded(i, w >> 2, t, XSO_TAG_SWEEP, run_seed, o);
-                    int R = (o[w & 3u] < w1_threshold) ? 1 : 0;
+                    uint64_t u = (uint64_t)o[w & 3u];
                     int k = unsat_count(i, nbr, cls, jbit, mode == 1 ? snap : s1);
-                    int flip = (k >= 2) || (k == 1 && R);
+                    int flip = (u < thr4[k]) ? 1 : 0;
                     if (!flip) continue;
                     if (check_dE) {
                         int32_t e0 = xso_energy(N, tri, jbit, s1);
@@ -307,6 +311,27 @@ void xso_sweep(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri
     free(snap);
 }
 
+/* The quasi-greedy table w = (0, w1, 1, 1) of L67 / L101. */
+static void qg_table(uint32_t w1_threshold, uint64_t thr4[4])
+{
+    thr4[0] = 0;
+    thr4[1] = (uint64_t)w1_threshold;
+    thr4[2] = (uint64_t)1 << 32;
+    thr4[3] = (uint64_t)1 << 32;
+}
+
+void xso_sweep(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri,
+               const uint8_t* jbit, const uint32_t* nbr, const uint32_t* cls,
+               const uint32_t* order, const uint32_t* set_size, uint32_t n_sets,
+               uint64_t run_seed, uint32_t t, uint32_t w1_threshold, int mode,
+               int check_dE, int8_t* s, uint64_t* n_flips, uint64_t* dE_mismatch)
+{
+    uint64_t thr4[4];
+    qg_table(w1_threshold, thr4);
+    xso_sweep_w(N, w_begin, w_end, tri, jbit, nbr, cls, order, set_size, n_sets, run_seed, t, thr4,
+                mode, check_dE, s, n_flips, dE_mismatch);
+}
+
 /* ---- run: sweeps t_begin+1 .. t_begin+n_sweeps over words [w_begin,w_end) ------------
  * After each sweep, E_c by FULL recomputation; first_hit[c] = t at the first sweep after
  * which E_c = -N (L293 "the exact iteration ... is saved", L111).  first_hit must be
@@ -321,20 +346,32 @@ void xso_mark_initial(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32
     }
 }
 
+void xso_run_w(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri,
+               const uint8_t* jbit, const uint32_t* nbr, const uint32_t* cls,
+               const uint32_t* order, const uint32_t* set_size, uint32_t n_sets,
+               uint64_t run_seed, uint32_t t_begin, uint32_t n_sweeps, const uint64_t* thr4,
+               int8_t* s, uint32_t* first_hit)
+{
+    for (uint32_t t = t_begin + 1u; t <= t_begin + n_sweeps; ++t) {
+        xso_sweep_w(N, w_begin, w_end, tri, jbit, nbr, cls, order, set_size, n_sets, run_seed,
+                    t, thr4, 0, 0, s, NULL, NULL);
+        for (size_t c = (size_t)64u * w_begin; c < (size_t)64u * w_end; ++c)
+            if (first_hit[c] == 0xFFFFFFFFu &&
+                xso_energy(N, tri, jbit, s + c * N) == -(int32_t)N)
+                first_hit[c] = t;
+    }
+}
+
 void xso_run(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri,
              const uint8_t* jbit, const uint32_t* nbr, const uint32_t* cls,
              const uint32_t* order, const uint32_t* set_size, uint32_t n_sets,
              uint64_t run_seed, uint32_t t_begin, uint32_t n_sweeps, uint32_t w1_threshold,
              int8_t* s, uint32_t* first_hit)
 {
-    for (uint32_t t = t_begin + 1u; t <= t_begin + n_sweeps; ++t) {
-        xso_sweep(N, w_begin, w_end, tri, jbit, nbr, cls, order, set_size, n_sets, run_seed,
-                  t, w1_threshold, 0, 0, s, NULL, NULL);
-        for (size_t c = (size_t)64u * w_begin; c < (size_t)64u * w_end; ++c)
-            if (first_hit[c] == 0xFFFFFFFFu &&
-                xso_energy(N, tri, jbit, s + c * N) == -(int32_t)N)
-                first_hit[c] = t;
-    }
+    uint64_t thr4[4];
+    qg_table(w1_threshold, thr4);
+    xso_run_w(N, w_begin, w_end, tri, jbit, nbr, cls, order, set_size, n_sets, run_seed, t_begin,
+              n_sweeps, thr4, s, first_hit);
 }
 
 /* Same as xso_run but words are distributed over OpenMP threads (words evolve

@@ -61,6 +61,12 @@ def lib():
                     C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, i8p, u32p]
         L.xso_run.argtypes = run_args
         L.xso_run_omp.argtypes = run_args
+        # general flip table w_0..w_3: thresholds in [0, 2^32] as uint64[4]
+        L.xso_sweep_w.argtypes = [C.c_uint32, C.c_uint32, C.c_uint32, u32p, u8p, u32p, u32p,
+                                  u32p, u32p, C.c_uint32, C.c_uint64, C.c_uint32, u64p,
+                                  C.c_int, C.c_int, i8p, u64p, u64p]
+        L.xso_run_w.argtypes = [C.c_uint32, C.c_uint32, C.c_uint32, u32p, u8p, u32p, u32p, u32p,
+                                u32p, C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32, u64p, i8p, u32p]
         L.xso_pack.argtypes = [C.c_uint32, C.c_uint32, i8p, u64p]
         L.xso_unpack.argtypes = [C.c_uint32, C.c_uint32, u64p, i8p]
         L.xso_omp_threads.restype = C.c_int
@@ -146,14 +152,23 @@ class Instance:
                         dtype=np.int32)
 
     def sweep(self, s, run_seed, t, w_begin=0, w_end=None, thr=W1_THRESHOLD, mode=0,
-              check_dE=False, order=None, set_size=None):
-        """One sweep number t (in place).  Returns (n_flips, dE_mismatches)."""
+              check_dE=False, order=None, set_size=None, thr4=None):
+        """One sweep number t (in place).  Returns (n_flips, dE_mismatches).
+        thr4: general flip table (4 thresholds in [0, 2^32]); default = quasi-greedy with `thr`."""
         assert s.dtype == np.int8 and s.flags.c_contiguous
         W = s.shape[0] // 64
         w_end = W if w_end is None else w_end
         order = self.order if order is None else np.ascontiguousarray(order, dtype=np.uint32)
         ss = self.set_size if set_size is None else np.ascontiguousarray(set_size, dtype=np.uint32)
         nf, mm = C.c_uint64(0), C.c_uint64(0)
+        if thr4 is not None:
+            t4 = np.ascontiguousarray(thr4, dtype=np.uint64)
+            lib().xso_sweep_w(self.N, w_begin, w_end, _p(self.tri, C.c_uint32),
+                              _p(self.jbit, C.c_uint8), _p(self.nbr, C.c_uint32),
+                              _p(self.cls, C.c_uint32), _p(order, C.c_uint32), _p(ss, C.c_uint32),
+                              len(ss), int(run_seed), int(t), _p(t4, C.c_uint64), int(mode),
+                              int(bool(check_dE)), _p(s, C.c_int8), C.byref(nf), C.byref(mm))
+            return nf.value, mm.value
         lib().xso_sweep(self.N, w_begin, w_end, _p(self.tri, C.c_uint32), _p(self.jbit, C.c_uint8),
                         _p(self.nbr, C.c_uint32), _p(self.cls, C.c_uint32),
                         _p(order, C.c_uint32), _p(ss, C.c_uint32), len(ss), int(run_seed),
@@ -170,12 +185,21 @@ class Instance:
         return fh
 
     def run(self, s, first_hit, run_seed, t_begin, n_sweeps, w_begin=0, w_end=None,
-            thr=W1_THRESHOLD, omp=False):
+            thr=W1_THRESHOLD, omp=False, thr4=None):
         """Sweeps t_begin+1 .. t_begin+n_sweeps in place, maintaining first_hit."""
         assert s.dtype == np.int8 and s.flags.c_contiguous
         assert first_hit.dtype == np.uint32 and first_hit.flags.c_contiguous
         W = s.shape[0] // 64
         w_end = W if w_end is None else w_end
+        if thr4 is not None:
+            t4 = np.ascontiguousarray(thr4, dtype=np.uint64)
+            lib().xso_run_w(self.N, w_begin, w_end, _p(self.tri, C.c_uint32),
+                            _p(self.jbit, C.c_uint8), _p(self.nbr, C.c_uint32),
+                            _p(self.cls, C.c_uint32), _p(self.order, C.c_uint32),
+                            _p(self.set_size, C.c_uint32), self.n_sets, int(run_seed),
+                            int(t_begin), int(n_sweeps), _p(t4, C.c_uint64), _p(s, C.c_int8),
+                            _p(first_hit, C.c_uint32))
+            return
         fn = lib().xso_run_omp if omp else lib().xso_run
         fn(self.N, w_begin, w_end, _p(self.tri, C.c_uint32), _p(self.jbit, C.c_uint8),
            _p(self.nbr, C.c_uint32), _p(self.cls, C.c_uint32), _p(self.order, C.c_uint32),

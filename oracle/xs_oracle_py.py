@@ -90,6 +90,18 @@ def energy(tri, J, s1):
     return -sum(J[t] * s1[i] * s1[j] * s1[k] for t, (i, j, k) in enumerate(tri))
 
 
+def sweep_table(N, W, adj, J, order, run_seed, t, thr4, s):
+    """L67, L69: flip with probability w_k = thr4[k] / 2^32, the same number for every k."""
+    for i in order:
+        for w in range(W):
+            u = _rng(i, w >> 2, t, SWEEP, run_seed)[w & 3]
+            for b in range(64):
+                s1 = s[64 * w + b]
+                k = sum(1 for (c, a, bb) in adj[i] if J[c] * s1[i] * s1[a] * s1[bb] == -1)
+                if u < thr4[k]:
+                    s1[i] = -s1[i]
+
+
 def sweep(N, W, adj, J, order, run_seed, t, thr, s):
     """L65-L67, L87, L101: w0 = 0, w1 = thr / 2^32, w2 = w3 = 1, one number per word."""
     for i in order:
