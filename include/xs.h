@@ -121,6 +121,16 @@ int xs_create_instance_from_arrays(xs_batch** out, const xs_params* p, const uin
  * per-instance solved / TTS records on the device.  Asynchronous on cuda_stream. */
 int xs_run_sweeps(xs_batch* b, uint64_t n_sweeps, void* cuda_stream);
 
+/* general flip table.  PAPER.md L67: w_k = probability of flipping a spin
+ * that enters k unsatisfied interactions; the quasi-greedy rule is w = (0, 0.055, 1, 1); L69:
+ * w0 = w1^3, w2 = w3 = 1 satisfies detailed balance (Metropolis at T = -2 / ln w1).
+ * thr4[k] in [0, 2^32] (host array): the spin flips iff the word's 32-bit number u < thr4[k];
+ * the same u serves every k (L87).  Takes effect from the next xs_run_sweeps; the default after
+ * xs_create_instance* is (0, w1_threshold, 2^32, 2^32).  Tables that are not of the quasi-greedy
+ * form run on the generic / streaming kernels; with thr4[0] > 0 a ground state can be left
+ * again, so first hits are looked for after every sweep.  Host call, no CUDA work. */
+int xs_set_flip_table(xs_batch* b, const uint64_t* thr4);
+
 /* a-11.  E_c = -sum_t J_t s_i s_j s_k (L41) for every clone: dev_out [inst][64 W] int32. */
 int xs_energy(xs_batch* b, int32_t* dev_out, void* cuda_stream);
 

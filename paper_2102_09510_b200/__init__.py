@@ -11,7 +11,7 @@ from ._binding import (XS_FLAG_GAUGE, XS_FLAG_NO_SKIP, XS_FLAG_STREAMING, XS_NO_
                        XS_W1_THRESHOLD_DEFAULT, XsError, lib, make_params, xs_alu_peak,
                        xs_create_instance, xs_kernel_launches,
                        xs_create_instance_from_arrays, xs_destroy, xs_energy, xs_get_first_hit,
-                       xs_generate_graph, xs_get_graph, xs_get_layout, xs_get_spins, xs_params, xs_run_sweeps,
+                       xs_generate_graph, xs_get_graph, xs_get_layout, xs_get_spins, xs_params, xs_run_sweeps, xs_set_flip_table,
                        xs_set_spins, xs_tts, xs_tts_rec, xs_tts_stats, xs_workspace_bytes)
 
 
@@ -47,6 +47,9 @@ class Batch:
     # -- calls, same names as the C ABI ------------------------------------------------------
     def run_sweeps(self, n_sweeps: int, stream=None):
         xs_run_sweeps(self.h, n_sweeps, stream)
+
+    def set_flip_table(self, thr4):
+        xs_set_flip_table(self.h, thr4)
 
     def energy(self, stream=None):
         import torch

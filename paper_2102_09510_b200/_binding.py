@@ -36,7 +36,7 @@ class xs_layout(C.Structure):
 
 
 EXPORTS = ["xs_workspace_bytes", "xs_create_instance", "xs_create_instance_from_arrays",
-           "xs_run_sweeps", "xs_energy", "xs_tts", "xs_get_spins", "xs_set_spins",
+           "xs_run_sweeps", "xs_set_flip_table", "xs_energy", "xs_tts", "xs_get_spins", "xs_set_spins",
            "xs_get_first_hit", "xs_get_graph", "xs_generate_graph", "xs_get_layout", "xs_tts_stats",
            "xs_alu_peak", "xs_kernel_launches", "xs_destroy",
            "xs_last_error"]
@@ -60,6 +60,7 @@ def lib():
     L.xs_create_instance_from_arrays.argtypes = [C.POINTER(vp), pp, u32p, u8p, u32p, u32p, u32p,
                                                  C.c_uint32, u64p, vp, C.c_size_t, vp]
     L.xs_run_sweeps.argtypes = [vp, C.c_uint64, vp]
+    L.xs_set_flip_table.argtypes = [vp, u64p]
     L.xs_energy.argtypes = [vp, vp, vp]
     L.xs_tts.argtypes = [vp, C.POINTER(xs_tts_rec), vp]
     L.xs_get_spins.argtypes = [vp, vp, vp]
@@ -153,6 +154,12 @@ def xs_create_instance_from_arrays(params: xs_params, tri, jbit, order, set_size
 
 def xs_run_sweeps(h, n_sweeps: int, stream=None):
     _check(lib().xs_run_sweeps(h, int(n_sweeps), _stream(stream)), "xs_run_sweeps")
+
+
+def xs_set_flip_table(h, thr4):
+    t = _np(thr4, np.uint64)
+    assert t.size == 4
+    _check(lib().xs_set_flip_table(h, _ptr(t, C.c_uint64)), "xs_set_flip_table")
 
 
 def xs_energy(h, dev_out_ptr: int, stream=None):

@@ -131,6 +131,8 @@ static int finish_create(xs_batch* b, void* dev_ws, size_t ws_bytes, void* strea
     // staging vectors die at return: make sure the copies are done
     if (cudaError_t e = cudaStreamSynchronize(st)) return cuda_fail((int)e, "upload sync");
 
+    // quasi-greedy table (0, w1, 1, 1) of L67 / L101 until xs_set_flip_table says otherwise
+    b->ft = FlipTable{{0u, p.w1_threshold, 0u, 0u}, 0xCu, 0u};
     std::string err;
     if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
     if (int e = launch_init(*b, stream)) return cuda_fail(e, "init kernel");
@@ -212,6 +214,24 @@ int xs_run_sweeps(xs_batch* b, uint64_t n_sweeps, void* cuda_stream)
     if (int e = launch_sweeps(*b, (uint32_t)n_sweeps, cuda_stream)) return cuda_fail(e, "sweep kernel");
     if (int e = launch_finalize(*b, (uint32_t)n_sweeps, cuda_stream)) return cuda_fail(e, "finalize kernel");
     b->sweeps_issued += n_sweeps;
+    return XS_OK;
+}
+
+int xs_set_flip_table(xs_batch* b, const uint64_t* thr4)
+{
+    if (!b || !thr4) return fail(XS_EINVAL, "null argument");
+    FlipTable ft{};
+    for (int k = 0; k < 4; ++k) {
+        if (thr4[k] > (1ull << 32)) return fail(XS_EINVAL, "threshold above 2^32");
+        if (thr4[k] == (1ull << 32)) ft.always |= 1u << k;
+        else ft.lo[k] = (uint32_t)thr4[k];
+    }
+    // the quasi-greedy form w = (0, w1 < 1, 1, 1) runs on the fast kernels
+    ft.general = !(thr4[0] == 0 && ft.always == 0xCu);
+    b->ft = ft;
+    if (!ft.general) b->p.w1_threshold = ft.lo[1];
+    std::string err;
+    if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
     return XS_OK;
 }
 

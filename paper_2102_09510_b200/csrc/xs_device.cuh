@@ -86,6 +86,25 @@ __device__ __forceinline__ uint32_t qg_update(uint32_t a0, uint32_t b0, uint32_t
     const uint32_t f = lop3<LUT_MAJ_NOTC>(M, P, x);
     return lop3<LUT_SEL>(R, f, M);
 }
+// General flip table (PAPER.md: w_k = probability of flipping a spin that enters k
+// unsatisfied interactions; L69: w0 = w1^3 gives detailed balance).  Rk = all-ones iff the
+// word's number is below the threshold of w_k.  k = 2 (M^x) + (P^x) selects the mask:
+//   flip = (M^x) ? ((P^x) ? R3 : R2) : ((P^x) ? R1 : R0)
+__device__ __forceinline__ uint32_t table_update(uint32_t a0, uint32_t b0, uint32_t j0, uint32_t a1,
+                                                 uint32_t b1, uint32_t j1, uint32_t a2, uint32_t b2,
+                                                 uint32_t j2, uint32_t x, uint32_t R0, uint32_t R1,
+                                                 uint32_t R2, uint32_t R3)
+{
+    const uint32_t w0 = lop3<LUT_XOR3>(a0, b0, j0);
+    const uint32_t w1 = lop3<LUT_XOR3>(a1, b1, j1);
+    const uint32_t w2 = lop3<LUT_XOR3>(a2, b2, j2);
+    const uint32_t Mu = lop3<LUT_MAJ>(w0, w1, w2) ^ x;
+    const uint32_t Pu = lop3<LUT_XOR3>(w0, w1, w2) ^ x;
+    const uint32_t lo = lop3<LUT_SEL>(Pu, R1, R0);
+    const uint32_t hi = lop3<LUT_SEL>(Pu, R3, R2);
+    return x ^ lop3<LUT_SEL>(Mu, hi, lo);
+}
+
 // Bits set where the spin has k != 0 unsatisfied clauses.
 __device__ __forceinline__ uint32_t qg_nonzero_k(uint32_t a0, uint32_t b0, uint32_t j0, uint32_t a1,
                                                  uint32_t b1, uint32_t j1, uint32_t a2, uint32_t b2,

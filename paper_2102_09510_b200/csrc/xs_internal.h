@@ -67,6 +67,15 @@ struct DevPtrs {
     uint32_t* n_sets;      // [I]
 };
 
+// Flip table w_0..w_3 as 32-bit thresholds: a spin with k unsatisfied
+// interactions flips iff bit k of `always` is set or the word's number u < lo[k].
+// general == 0: the quasi-greedy form (0, lo[1], 1, 1) -> the fast kernels apply.
+struct FlipTable {
+    uint32_t lo[4];
+    uint32_t always;
+    uint32_t general;
+};
+
 struct TileGeom {
     uint32_t regime = 0;       // 0 on-chip, 1 streaming
     uint32_t T = 0;            // uint64 columns per tile
@@ -88,6 +97,7 @@ struct xs_batch {
     xs::DevLayout lay;
     xs::DevPtrs d{};
     xs::TileGeom geom;
+    xs::FlipTable ft{};
     uint32_t n_sets_max = 0;
     uint32_t max_set_size = 0;
     uint64_t sweeps_issued = 0;   // upper bound on any instance's sweep counter (overflow guard)

@@ -201,6 +201,7 @@ __global__ void __launch_bounds__(256) k_finalize(DevPtrs d, uint32_t W, uint32_
 // ------------------------------------------------------------------------------------------
 struct TileArgs {
     DevPtrs d;
+    FlipTable ft;
     uint32_t N, W, T, n_sweeps, thr, flags, batch, rb;
     uint32_t off_rec, off_rbuf, off_sets, off_misc;   // byte offsets in dynamic shared memory
 };
@@ -239,7 +240,7 @@ __device__ __forceinline__ void tile_gather(const TileCtx<CW>& c, uint32_t p, ui
 }
 
 // one sweep over all sets, sweep slot `rs` of the random-byte ring
-template <int CW>
+template <int CW, bool GEN>
 __device__ __forceinline__ void tile_sweep(const TileCtx<CW>& c, uint32_t rs)
 {
     const unsigned char* rb = c.rbuf + (size_t)rs * c.N * c.T + c.jw;
@@ -248,19 +249,30 @@ __device__ __forceinline__ void tile_sweep(const TileCtx<CW>& c, uint32_t rs)
         for (uint32_t p = c.sets[s] + c.slot; p < p1; p += c.n_slots) {
             uint32_t a[3][2 * CW], b[3][2 * CW], x[2 * CW], jm[3], self_off;
             tile_gather<CW>(c, p, a, b, x, jm, self_off);
-            uint32_t R[CW];
+            uint32_t nb[CW];          // noise byte of each word
             if (CW == 2) {
                 const uint32_t two = *reinterpret_cast<const unsigned short*>(rb + (size_t)p * c.T);
-                R[0] = (uint32_t)(int32_t)(int8_t)(two & 0xFF);
-                R[CW - 1] = (uint32_t)(int32_t)(int8_t)(two >> 8);
+                nb[0] = two & 0xFFu;
+                nb[CW - 1] = two >> 8;
             } else {
-                R[0] = (uint32_t)(int32_t)(int8_t)rb[(size_t)p * c.T];
+                nb[0] = rb[(size_t)p * c.T];
             }
             uint32_t xn[2 * CW];
+            if (GEN) {
+                // general table: bit k of the byte <=> number below the threshold of w_k
 #pragma unroll
-            for (int h = 0; h < 2 * CW; ++h)
-                xn[h] = qg_update(a[0][h], b[0][h], jm[0], a[1][h], b[1][h], jm[1], a[2][h], b[2][h],
-                                  jm[2], x[h], R[h >> 1]);
+                for (int h = 0; h < 2 * CW; ++h) {
+                    const uint32_t v = nb[h >> 1];
+                    xn[h] = table_update(a[0][h], b[0][h], jm[0], a[1][h], b[1][h], jm[1], a[2][h],
+                                         b[2][h], jm[2], x[h], 0u - (v & 1u), 0u - ((v >> 1) & 1u),
+                                         0u - ((v >> 2) & 1u), 0u - ((v >> 3) & 1u));
+                }
+            } else {
+#pragma unroll
+                for (int h = 0; h < 2 * CW; ++h)
+                    xn[h] = qg_update(a[0][h], b[0][h], jm[0], a[1][h], b[1][h], jm[1], a[2][h], b[2][h],
+                                      jm[2], x[h], (uint32_t)(int32_t)(int8_t)nb[h >> 1]);
+            }
             vstore<CW>(c.state + self_off + c.joff, xn);
         }
         __syncthreads();
@@ -292,8 +304,19 @@ __device__ __forceinline__ void tile_detect_acc(const TileCtx<CW>& c)
 // position, group of 4 words); round keys precomputed; G is a power of two (no divisions).
 template <int CW>
 __device__ __forceinline__ void tile_produce(const TileCtx<CW>& c, uint32_t t_first, uint32_t ns,
-                                             uint32_t w0, const uint32_t (&ks)[10][2], uint32_t thr)
+                                             uint32_t w0, const uint32_t (&ks)[10][2],
+                                             const FlipTable& ft)
 {
+    const uint32_t thr = ft.lo[1];
+    // noise byte of one word: quasi-greedy 0xFF / 0x00 (k = 1 threshold); general table: bit k
+    auto nbyte = [&](uint32_t u) -> uint32_t {
+        if (!ft.general) return u < thr ? 0xFFu : 0u;
+        uint32_t v = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            v |= ((((ft.always >> k) & 1u) != 0u) || (u < ft.lo[k])) ? (1u << k) : 0u;
+        return v;
+    };
     const uint32_t G = c.T >= 4 ? c.T / 4 : 1;
     const uint32_t gsh = (uint32_t)__ffs((int)G) - 1u;
     const uint32_t per_sweep = c.N << gsh;
@@ -308,12 +331,12 @@ __device__ __forceinline__ void tile_produce(const TileCtx<CW>& c, uint32_t t_fi
             philox4x32_10_ks(spin, grp0 + g, t, TAG_SWEEP, ks, o);
             unsigned char* dst = row + (size_t)p * c.T;
             if (c.T >= 4) {
-                const uint32_t v = (o[0] < thr ? 0xFFu : 0u) | (o[1] < thr ? 0xFF00u : 0u) |
-                                   (o[2] < thr ? 0xFF0000u : 0u) | (o[3] < thr ? 0xFF000000u : 0u);
+                const uint32_t v = nbyte(o[0]) | (nbyte(o[1]) << 8) | (nbyte(o[2]) << 16) |
+                                   (nbyte(o[3]) << 24);
                 *reinterpret_cast<uint32_t*>(dst + 4 * g) = v;
             } else {
                 for (uint32_t lw = 0; lw < c.T; ++lw)
-                    dst[lw] = o[(w0 + lw) & 3u] < thr ? 0xFF : 0;
+                    dst[lw] = (unsigned char)nbyte(o[(w0 + lw) & 3u]);
             }
         }
     }
@@ -402,10 +425,10 @@ __global__ void __launch_bounds__(1024, 1) k_sweep_tile(TileArgs A)
     auto run_range = [&](uint32_t t0, uint32_t n, bool exact) {
         for (uint32_t s0 = 0; s0 < n; s0 += A.rb) {
             const uint32_t ns = min(A.rb, n - s0);
-            tile_produce<CW>(c, t0 + s0 + 1, ns, w0, ks, A.thr);
+            tile_produce<CW>(c, t0 + s0 + 1, ns, w0, ks, A.ft);
             __syncthreads();
             for (uint32_t s = 0; s < ns; ++s) {
-                tile_sweep<CW>(c, s);
+                if (A.ft.general) tile_sweep<CW, true>(c, s); else tile_sweep<CW, false>(c, s);
                 if (exact) {
                     detect();
                     const uint32_t t = t0 + s0 + s + 1;
@@ -428,17 +451,23 @@ __global__ void __launch_bounds__(1024, 1) k_sweep_tile(TileArgs A)
     uint32_t remaining = A.n_sweeps;
     while (remaining) {
         const uint32_t nb = min(A.batch, remaining);
-        run_range(t, nb, false);
-        detect();
-        for (uint32_t e = threadIdx.x; e < 2 * T; e += blockDim.x)
-            if (~c.det32[e] & ~c.known32[e]) *c.flag = 1;
-        __syncthreads();
-        const bool replay = *c.flag != 0;
-        __syncthreads();
-        if (replay) {
-            load_state();          // global copy = state at the start of this batch
-            __syncthreads();
+        if (A.ft.lo[0] != 0u || (A.ft.always & 1u)) {
+            // w0 > 0: a ground state can be left again (L69), so the batch-end check could miss
+            // a visit -> check after every sweep
             run_range(t, nb, true);
+        } else {
+            run_range(t, nb, false);
+            detect();
+            for (uint32_t e = threadIdx.x; e < 2 * T; e += blockDim.x)
+                if (~c.det32[e] & ~c.known32[e]) *c.flag = 1;
+            __syncthreads();
+            const bool replay = *c.flag != 0;
+            __syncthreads();
+            if (replay) {
+                load_state();          // global copy = state at the start of this batch
+                __syncthreads();
+                run_range(t, nb, true);
+            }
         }
         store_state();             // a-10 (also the replay checkpoint of the next batch)
         t += nb;
@@ -459,9 +488,10 @@ constexpr uint32_t ST_THREADS = 256;
 template <int CW>
 __global__ void __launch_bounds__(ST_THREADS) k_stream_set(DevPtrs d, uint32_t N, uint32_t W,
                                                           uint32_t set_idx, uint32_t s_rel,
-                                                          uint32_t thr, uint32_t flags, uint64_t* det)
+                                                          FlipTable ft, uint32_t flags, uint64_t* det)
 {
     __shared__ uint32_t sdet[1024];
+    const uint32_t thr = ft.lo[1];
     const uint32_t inst = blockIdx.y;
     const xs_tts_rec rec = d.rec[inst];
     if (rec.solved && !(flags & XS_FLAG_NO_SKIP)) return;
@@ -510,11 +540,21 @@ __global__ void __launch_bounds__(ST_THREADS) k_stream_set(DevPtrs d, uint32_t N
         uint32_t xn[2 * CW];
 #pragma unroll
         for (int h = 0; h < 2 * CW; ++h) {
-            const uint32_t R = o[(w + (h >> 1)) & 3u] < thr ? ~0u : 0u;
+            const uint32_t u = (((w + (h >> 1)) & 3u) == 0u) ? o[0] : (((w + (h >> 1)) & 3u) == 1u) ? o[1]
+                               : (((w + (h >> 1)) & 3u) == 2u) ? o[2] : o[3];
             const uint32_t nz = qg_nonzero_k(a[0][h], b[0][h], jm0, a[1][h], b[1][h], jm1, a[2][h],
                                              b[2][h], jm2, xo[h]);
-            xn[h] = qg_update(a[0][h], b[0][h], jm0, a[1][h], b[1][h], jm1, a[2][h], b[2][h], jm2,
-                              xo[h], R);
+            if (ft.general) {
+                uint32_t Rk[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    Rk[k] = ((((ft.always >> k) & 1u) != 0u) || (u < ft.lo[k])) ? ~0u : 0u;
+                xn[h] = table_update(a[0][h], b[0][h], jm0, a[1][h], b[1][h], jm1, a[2][h], b[2][h],
+                                     jm2, xo[h], Rk[0], Rk[1], Rk[2], Rk[3]);
+            } else {
+                xn[h] = qg_update(a[0][h], b[0][h], jm0, a[1][h], b[1][h], jm1, a[2][h], b[2][h], jm2,
+                                  xo[h], u < thr ? ~0u : 0u);
+            }
             if (fixed) acc[h] |= nz;
             else if (nz) atomicOr(&det32[2 * w + h], nz);
         }
@@ -616,7 +656,7 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     // 1) static-task kernel (xs_sweep_static.cu): work list in registers, T in {8,16,32,64}
     // many small tiles (e.g. 20,000 runs of W = 4): the generic kernel's high occupancy wins
     const bool few_tiles = (uint64_t)p.n_instances * ((p.n_words + 7) / 8) < 2ull * NUM_SMS;
-    if (!(p.flags & XS_FLAG_STREAMING) &&
+    if (!(p.flags & XS_FLAG_STREAMING) && !b.ft.general &&     // static kernel: quasi-greedy table only
         (want_variant == 1 || (want_variant == 2 && !auto_T && few_tiles))) {
         const uint32_t force_thr = env_u32("XS_THREADS", 0);
         const uint32_t force_cw = env_u32("XS_CW", 0);
@@ -795,6 +835,7 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
         A.d = b.d;
         A.N = p.n_spins; A.W = p.n_words; A.T = g.T; A.n_sweeps = n_sweeps;
         A.thr = p.w1_threshold; A.flags = p.flags; A.batch = g.batch; A.rb = g.rb;
+        A.ft = b.ft;
         A.off_rec = s.off_rec; A.off_rbuf = s.off_rbuf; A.off_sets = s.off_sets; A.off_misc = s.off_misc;
         if (g.CW == 2) {
             XS_CU(cudaFuncSetAttribute(k_sweep_tile<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.total));
@@ -818,15 +859,25 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
         for (uint32_t set = 0; set < b.n_sets_max; ++set) {
             if (g.CW == 2)
                 k_stream_set<2><<<grid, ST_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, set, s,
-                                                             p.w1_threshold, p.flags, cur);
+                                                             b.ft, p.flags, cur);
             else
                 k_stream_set<1><<<grid, ST_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, set, s,
-                                                             p.w1_threshold, p.flags, cur);
+                                                             b.ft, p.flags, cur);
             count_launch(1);
         }
-        k_stream_commit<<<grid_for(clones, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, cur,
-                                                              det[(s + 1) & 1], s, p.flags);
-        count_launch(1);
+        if (b.ft.lo[0] != 0u || (b.ft.always & 1u)) {
+            // w0 > 0: ground states are not absorbing (L69): look at the state after every sweep
+            int rc = launch_unsat_or(b, st);
+            if (rc) return rc;
+            k_mark_swept<<<grid_for(clones, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, b.d.det,
+                                                               s, p.flags);
+            count_launch(1);
+            XS_CU(cudaMemsetAsync(b.d.det, 0, 2 * det_words * 8, st));
+        } else {
+            k_stream_commit<<<grid_for(clones, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, cur,
+                                                                  det[(s + 1) & 1], s, p.flags);
+            count_launch(1);
+        }
         XS_CU(cudaGetLastError());
     }
     int rc = launch_unsat_or(b, st);

@@ -15,9 +15,10 @@ class OracleRun:
     instance was already solved at call entry (and skipping is on)."""
 
     def __init__(self, N, W, graph_seed, run_seed, gauge=True, set_cap=0, thr=W1_THRESHOLD,
-                 no_skip=False, inst: Instance | None = None, words=None):
+                 no_skip=False, inst: Instance | None = None, words=None, thr4=None):
         self.inst = inst if inst is not None else Instance(N, graph_seed, gauge, set_cap)
         self.N, self.W, self.run_seed, self.thr, self.no_skip = N, W, run_seed, thr, no_skip
+        self.thr4 = thr4                     # general flip table (PAPER.md L67, L69) or None = QG
         # `words`: evolve only this subset of word indices (others stay at their initial value)
         self.words = list(range(W)) if words is None else sorted(words)
         self.s = self.inst.init_spins(W, run_seed)
@@ -37,7 +38,7 @@ class OracleRun:
             return
         for w in self.words:
             self.inst.run(self.s, self.first_hit, self.run_seed, self.sweeps_done, n, w, w + 1,
-                          thr=self.thr)
+                          thr=self.thr, thr4=self.thr4)
         self.sweeps_done += n
 
     def x(self) -> np.ndarray:
