@@ -21,12 +21,13 @@ import time
 import numpy as np
 
 
-def run_size(n, words, instances, runs, cap, chunk, seed0, flags_extra=0):
+def run_size(n, words, instances, runs, cap, chunk, seed0, flags_extra=0, w1=None):
     import torch
     import paper_2102_09510_b200 as xs
     gseeds = [seed0 + i for i in range(instances) for _ in range(runs)]
     rseeds = [seed0 + i + 7919 * (r + 1) for i in range(instances) for r in range(runs)]
-    b = xs.Batch(n, words, gseeds, rseeds, flags=xs.XS_FLAG_GAUGE | flags_extra)
+    thr = xs.XS_W1_THRESHOLD_DEFAULT if w1 is None else int(math.floor(w1 * 2.0 ** 32))
+    b = xs.Batch(n, words, gseeds, rseeds, flags=xs.XS_FLAG_GAUGE | flags_extra, w1_threshold=thr)
     lay = b.layout()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     done = 0
@@ -80,7 +81,7 @@ def run_size(n, words, instances, runs, cap, chunk, seed0, flags_extra=0):
     med = lambda a: float(np.median(a)) if np.isfinite(np.median(a)) else None   # noqa: E731
     lower = [s["tau_q16"] for s in per_inst if s["n_solved"] == 0]
     out = {
-        "n_spins": n, "clones": clones, "instances": instances, "runs_per_instance": runs,
+        "n_spins": n, "w1": (thr / 2.0 ** 32), "clones": clones, "instances": instances, "runs_per_instance": runs,
         "cap_sweeps": cap, "chunk": chunk, "regime": lay.regime, "tile_words": lay.tile_words,
         "solved_runs": n_solved_runs, "total_runs": instances * runs, "instances_with_a_solved_run": solved_inst,
         "median_tau_sweeps": med(taus), "median_tts99_sweeps": med(tts99),
@@ -118,12 +119,20 @@ def main():
     ap.add_argument("--cap", type=int, default=200000)
     ap.add_argument("--chunk", type=int, default=100)
     ap.add_argument("--seed0", type=int, default=100)
+    ap.add_argument("--w1", type=float, nargs="*", default=None,
+                    help="scan of w1 (PAPER.md Fig. 1, L91/L101: optimum 0.054(1)); default 0.055")
     args = ap.parse_args()
     rows = []
     for n in args.n:
-        r = run_size(n, args.words, args.instances, args.runs, args.cap, args.chunk, args.seed0)
-        rows.append(r)
-        print(json.dumps(r), flush=True)
+        for w1 in (args.w1 or [None]):
+            r = run_size(n, args.words, args.instances, args.runs, args.cap, args.chunk, args.seed0, w1=w1)
+            rows.append(r)
+            print(json.dumps(r), flush=True)
+    if args.w1:
+        best = min((r for r in rows if r["median_tau_sweeps"]), key=lambda r: r["median_tau_sweeps"])
+        print(json.dumps({"w1_scan": [[round(r["w1"], 4), r["median_tau_sweeps"]] for r in rows],
+                          "best_w1": best["w1"], "paper_optimum": "0.054(1), instance #38, N=256"}), flush=True)
+        return
     # exponential growth of the typical time with N (L151: TTS_99 ~ exp(a N), a = 0.0786(4))
     pts = [(r["n_spins"], math.log(r["median_tau_sweeps"] * r["clones"])) for r in rows
            if r["median_tau_sweeps"]]
