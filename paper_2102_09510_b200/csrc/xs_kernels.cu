@@ -641,7 +641,6 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     g.batch = std::max(1u, env_u32("XS_BATCH", 64));
     const uint32_t force_T = env_u32("XS_TILE_WORDS", 0);
     uint32_t bestT = 0;
-    uint64_t best_cost = ~0ull;
     // Measured on B200: with at least one 16-column tile per SM
     // the generic kernel with T = 16 (128-byte rows: conflict-free, several CTAs per SM overlap
     // their load / compute / barrier phases) is the fastest choice; with fewer tiles than SMs
@@ -712,7 +711,6 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
         }
         for (uint32_t T = 1; T <= 64 && !bestT; T <<= 1)
             if (ok(T)) bestT = T;
-        (void)best_cost;
     }
     if (bestT == 0) {
         g.regime = 1;
