@@ -98,7 +98,7 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def cpu_oracle_rate(wl, target_s: float = 12.0):
+def cpu_oracle_rate(wl, target_s: float = 20.0):
     """The oracle as it stands, OpenMP over words, on a bounded sample of the workload."""
     from oracle.xs_oracle import NO_HIT, Instance, omp_threads
     cores = omp_threads()
