@@ -485,12 +485,23 @@ __global__ void __launch_bounds__(1024, 1) k_sweep_tile(TileArgs A)
 // ------------------------------------------------------------------------------------------
 constexpr uint32_t ST_THREADS = 256;
 
+// Programmatic dependent launch: the streaming regime is a chain of short dependent launches
+// (one per independent set).  Launched with programmatic stream serialization, a kernel may
+// start while its predecessor drains; it must wait here before touching anything the
+// predecessor wrote, and lets its own successor start launching right away.
+__device__ __forceinline__ void pdl_wait_and_release()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 template <int CW>
 __global__ void __launch_bounds__(ST_THREADS) k_stream_set(DevPtrs d, uint32_t N, uint32_t W,
                                                           uint32_t set_idx, uint32_t s_rel,
                                                           FlipTable ft, uint32_t flags, uint64_t* det)
 {
     __shared__ uint32_t sdet[1024];
+    pdl_wait_and_release();
     const uint32_t thr = ft.lo[1];
     const uint32_t inst = blockIdx.y;
     const xs_tts_rec rec = d.rec[inst];
@@ -576,6 +587,7 @@ __global__ void __launch_bounds__(ST_THREADS) k_stream_set(DevPtrs d, uint32_t N
 __global__ void k_stream_commit(DevPtrs d, uint32_t W, uint32_t I, const uint64_t* det_cur,
                                 uint64_t* det_next, uint32_t s_rel, uint32_t flags)
 {
+    pdl_wait_and_release();
     const uint64_t total = (uint64_t)I * W * 64;
     for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
          e += (uint64_t)gridDim.x * blockDim.x) {
@@ -852,15 +864,24 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
     XS_CU(cudaMemsetAsync(b.d.det, 0, 2 * det_words * 8, st));
     dim3 grid(g.ctas, p.n_instances);
     const uint64_t clones = det_words * 64;
+    cudaLaunchAttribute pdl_attr[1];
+    pdl_attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    pdl_attr[0].val.programmaticStreamSerializationAllowed = 1;
     for (uint32_t s = 1; s <= n_sweeps; ++s) {
         uint64_t* cur = det[s & 1];
         for (uint32_t set = 0; set < b.n_sets_max; ++set) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = grid;
+            cfg.blockDim = dim3(ST_THREADS);
+            cfg.stream = st;
+            cfg.attrs = pdl_attr;
+            cfg.numAttrs = 1;
             if (g.CW == 2)
-                k_stream_set<2><<<grid, ST_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, set, s,
-                                                             b.ft, p.flags, cur);
+                XS_CU(cudaLaunchKernelEx(&cfg, k_stream_set<2>, b.d, p.n_spins, p.n_words, set, s, b.ft,
+                                         p.flags, cur));
             else
-                k_stream_set<1><<<grid, ST_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, set, s,
-                                                             b.ft, p.flags, cur);
+                XS_CU(cudaLaunchKernelEx(&cfg, k_stream_set<1>, b.d, p.n_spins, p.n_words, set, s, b.ft,
+                                         p.flags, cur));
             count_launch(1);
         }
         if (b.ft.lo[0] != 0u || (b.ft.always & 1u)) {
@@ -872,8 +893,14 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
             count_launch(1);
             XS_CU(cudaMemsetAsync(b.d.det, 0, 2 * det_words * 8, st));
         } else {
-            k_stream_commit<<<grid_for(clones, 256), 256, 0, st>>>(b.d, p.n_words, p.n_instances, cur,
-                                                                  det[(s + 1) & 1], s, p.flags);
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(grid_for(clones, 256));
+            cfg.blockDim = dim3(256);
+            cfg.stream = st;
+            cfg.attrs = pdl_attr;
+            cfg.numAttrs = 1;
+            XS_CU(cudaLaunchKernelEx(&cfg, k_stream_commit, b.d, p.n_words, p.n_instances,
+                                     (const uint64_t*)cur, det[(s + 1) & 1], s, p.flags));
             count_launch(1);
         }
         XS_CU(cudaGetLastError());
