@@ -32,8 +32,13 @@ if ROOT not in sys.path:
 
 # BASELINE.json configs[1]
 WORKLOADS = {
-    "config2": dict(N=256, W=1024, I=1, sweeps=10_000, graph_seed=2, run_seed=2,
-                    desc="configs[1]: N=256, 1 instance (graph seed 2), 2^16 clones, 10^4 sweeps, no early stop"),
+    # balanced independent sets of 64 = the slot count of the static kernel's CTA (DESIGN.md R-balance)
+    "config2": dict(N=256, W=1024, I=1, sweeps=10_000, graph_seed=2, run_seed=2, balanced=True, set_cap=64,
+                    desc="configs[1]: N=256, 1 instance (graph seed 2), 2^16 clones, 10^4 sweeps, no early stop; "
+                         "update order = 4 balanced independent sets of 64"),
+    "config2_greedy": dict(N=256, W=1024, I=1, sweeps=10_000, graph_seed=2, run_seed=2,
+                           desc="configs[1] with the uncapped greedy sets (61,62,59,50,23,1): N=256, 1 instance "
+                                "(graph seed 2), 2^16 clones, 10^4 sweeps, no early stop"),
     "config5": dict(N=1 << 20, W=16, I=1, sweeps=100, graph_seed=5, run_seed=5,
                     desc="configs[4]: N=2^20, 1 instance (graph seed 5), 2^10 clones, 100 sweeps (streaming)"),
     "config3": dict(N=512, W=64, I=256, sweeps=2_000, graph_seed=100, run_seed=100,
@@ -51,7 +56,7 @@ STREAM_BYTES_PER_UPDATE = (8 * 8 * 16 + 28) / 1024.0   # config 5, W=16: 1052 B 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu
 # --set full captures summarised in profiles/r01_ncu_summary.md (config5: the launch of the
 # largest independent set, 262,053 spin rows = 275.7 MB algorithmic).
-NCU_DRAM_BYTES_PER_LAUNCH = {"config2": 2.43e6, "config3": 91.6e6, "config5": 187.9e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"config2": 2.43e6, "config2_greedy": 2.43e6, "config3": 91.6e6, "config5": 187.9e6}
 
 
 class ClockSampler:
@@ -103,7 +108,7 @@ def cpu_oracle_rate(wl, target_s: float = 20.0):
     from oracle.xs_oracle import NO_HIT, Instance, omp_threads
     cores = omp_threads()
     N = wl["N"]
-    inst = Instance(N, wl["graph_seed"], True, 0)
+    inst = Instance(N, wl["graph_seed"], True, wl.get("set_cap", 0), balanced=bool(wl.get("balanced")))
     W = max(1, min(wl["W"], 4 * cores))      # enough words for ~target_s of work on all cores
     s = inst.init_spins(W, wl["run_seed"])
     fh = np.full(64 * W, NO_HIT, np.uint32)
@@ -176,7 +181,8 @@ def main():
     gseeds = [wl["graph_seed"] + i for i in range(I)]
     from paper_2102_09510_b200 import replicas
     rseeds = replicas.replica_run_seeds([wl["run_seed"] + i for i in range(I)], rank)   # replicas (L87)
-    b = xs.Batch(N, W, gseeds, rseeds, flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP, device=dev)
+    flags = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_BALANCED if wl.get("balanced") else 0)
+    b = xs.Batch(N, W, gseeds, rseeds, set_cap=wl.get("set_cap", 0), flags=flags, device=dev)
     lay = b.layout()
     updates_per_step = float(N) * 64.0 * W * I * sweeps
 

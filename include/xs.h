@@ -53,6 +53,13 @@ extern "C" {
                                     flag is set at call entry is skipped (L129/L293 stop rule)          */
 #define XS_FLAG_STREAMING    4u  /* force the streaming (global-memory) regime even if a tile fits
                                     on chip; the regimes are bit-identical (tests use this)             */
+#define XS_FLAG_BALANCED     8u  /* generated instances: balanced independent sets instead of the
+                                    greedy ones (L281: sets sized to keep the lanes evenly busy).
+                                    q = max(4, ceil(N / S)) sets of equal size (within one), S =
+                                    set_cap (0 -> 64), found by a deterministic tabu search seeded by
+                                    the graph seed (DESIGN.md R-balance); if the search fails the
+                                    greedy sets are used.  A different, equally valid update order:
+                                    trajectories differ from the greedy order's                         */
 
 /* w1 = 0.055 (L101) as a 32-bit threshold: flip a k=1 spin iff u32 < floor(0.055 * 2^32). */
 #define XS_W1_THRESHOLD_DEFAULT 236223201u
@@ -153,7 +160,7 @@ int xs_get_graph(const xs_batch* b, uint32_t inst, uint32_t* tri, uint8_t* jbit,
 /* a-1 alone, host only (no CUDA work): builds one instance from graph_seed exactly as
  * xs_create_instance does and writes tri [N][3], jbit [N], order [N], set_size [N] (first
  * *n_sets entries valid), *attempt = index of the accepted configuration-model attempt.
- * Any output pointer may be NULL.  flags: only XS_FLAG_GAUGE is looked at. */
+ * Any output pointer may be NULL.  flags: only XS_FLAG_GAUGE and XS_FLAG_BALANCED are looked at. */
 int xs_generate_graph(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uint32_t set_cap,
                       uint32_t* tri, uint8_t* jbit, uint32_t* order, uint32_t* set_size,
                       uint32_t* n_sets, int32_t* attempt);

@@ -191,6 +191,94 @@ int xso_update_order(uint32_t N, const uint32_t* nbr, uint32_t cap, uint32_t* or
     return (int)n_sets;
 }
 
+/* ---- update order, balanced variant (L281: sets sized "to keep the processing of components
+ * as balanced as possible"; DESIGN.md R-balance) ---------------------------------------------
+ * q sets of equal size (within one), found by a tabu search over colour swaps.  Every step is
+ * integer and deterministic:
+ *   col[i] = i mod q;  cnt[v][c] = number of the 6 entries nbr[v][.] with colour c;
+ *   conf = sum_v cnt[v][col[v]];  best = conf;  tabu[v][c] = 0.
+ *   for it = 1 .. max_it, while conf > 0:
+ *     L = spins with cnt[v][col[v]] > 0, ascending;  rnd = Philox(ctr=(it,0,0,5), key=seed);
+ *     v = L[rnd[0] mod |L|], a = col[v];
+ *     among all u (ascending) with b = col[u] != a, m = multiplicity of u in nbr[v][.]:
+ *         d = cnt[v][b] - cnt[v][a] + cnt[u][a] - cnt[u][b] - 2m      (change of conf / 2)
+ *         u is skipped if (tabu[v][b] >= it or tabu[u][a] >= it) and not conf + 2d < best;
+ *         keep the first u with the smallest d;
+ *     none: next it.  Else swap the colours of v and u, update cnt of their neighbours,
+ *     conf += 2d, tabu[v][a] = it + 5 + rnd[1] mod 10, tabu[u][b] = it + 5 + rnd[2] mod 10,
+ *     best = min(best, conf).
+ * conf == 0: set c = the spins of colour c in ascending order, sets in colour order; returns q.
+ * Otherwise (or if q < 2 or q > N) returns 0 and the caller uses the greedy order. */
+#define XSO_TAG_PARTITION 5u
+int xso_balanced_order(uint32_t N, const uint32_t* nbr, uint64_t seed, uint32_t q,
+                       uint32_t max_it, uint32_t* order, uint32_t* set_size)
+{
+    if (q < 2u || q > N) return 0;
+    uint32_t* col = (uint32_t*)malloc(sizeof(uint32_t) * N);
+    int32_t* cnt = (int32_t*)calloc((size_t)N * q, sizeof(int32_t));
+    uint32_t* tabu = (uint32_t*)calloc((size_t)N * q, sizeof(uint32_t));
+    uint32_t* L = (uint32_t*)malloc(sizeof(uint32_t) * N);
+    if (!col || !cnt || !tabu || !L) { free(col); free(cnt); free(tabu); free(L); return -1; }
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    for (uint32_t i = 0; i < N; ++i) col[i] = i % q;
+    for (uint32_t v = 0; v < N; ++v)
+        for (int k = 0; k < 6; ++k) cnt[(size_t)v * q + col[nbr[6 * v + k]]] += 1;
+    int64_t conf = 0;
+    for (uint32_t v = 0; v < N; ++v) conf += cnt[(size_t)v * q + col[v]];
+    int64_t best = conf;
+    for (uint32_t it = 1; it <= max_it && conf > 0; ++it) {
+        uint32_t nL = 0;
+        for (uint32_t v = 0; v < N; ++v)
+            if (cnt[(size_t)v * q + col[v]] > 0) L[nL++] = v;
+        const uint32_t ctr[4] = { it, 0u, 0u, XSO_TAG_PARTITION };
+        uint32_t rnd[4];
+        xso_philox4x32_10(ctr, key, rnd);
+        const uint32_t v = L[rnd[0] % nL], a = col[v];
+        int found = 0;
+        uint32_t bu = 0;
+        int32_t bd = 0;
+        for (uint32_t u = 0; u < N; ++u) {
+            const uint32_t b = col[u];
+            if (b == a) continue;
+            int32_t m = 0;
+            for (int k = 0; k < 6; ++k) m += (nbr[6 * v + k] == u);
+            const int32_t d = cnt[(size_t)v * q + b] - cnt[(size_t)v * q + a] +
+                              cnt[(size_t)u * q + a] - cnt[(size_t)u * q + b] - 2 * m;
+            const int is_tabu = tabu[(size_t)v * q + b] >= it || tabu[(size_t)u * q + a] >= it;
+            if (is_tabu && !(conf + 2 * (int64_t)d < best)) continue;
+            if (!found || d < bd) { found = 1; bu = u; bd = d; }
+        }
+        if (!found) continue;
+        const uint32_t u = bu, b = col[u];
+        for (int k = 0; k < 6; ++k) {
+            const uint32_t w = nbr[6 * v + k];
+            cnt[(size_t)w * q + a] -= 1; cnt[(size_t)w * q + b] += 1;
+        }
+        for (int k = 0; k < 6; ++k) {
+            const uint32_t w = nbr[6 * u + k];
+            cnt[(size_t)w * q + b] -= 1; cnt[(size_t)w * q + a] += 1;
+        }
+        col[v] = b; col[u] = a;
+        conf += 2 * (int64_t)bd;
+        tabu[(size_t)v * q + a] = it + 5u + rnd[1] % 10u;
+        tabu[(size_t)u * q + b] = it + 5u + rnd[2] % 10u;
+        if (conf < best) best = conf;
+    }
+    int rc = 0;
+    if (conf == 0) {
+        uint32_t p = 0;
+        for (uint32_t c = 0; c < q; ++c) {
+            uint32_t sz = 0;
+            for (uint32_t v = 0; v < N; ++v)
+                if (col[v] == c) { order[p++] = v; ++sz; }
+            set_size[c] = sz;
+        }
+        rc = (int)q;
+    }
+    free(col); free(cnt); free(tabu); free(L);
+    return rc;
+}
+
 /* 1 if every set is an anti-clique (no member is a neighbour of another member) and
  * order is a permutation of 0..N-1; else 0.  (L277: "nodes that are not directly
  * connected can be processed in parallel") */

@@ -47,6 +47,9 @@ def lib():
         L.xso_adjacency.restype = C.c_int
         L.xso_update_order.argtypes = [C.c_uint32, u32p, C.c_uint32, u32p, u32p]
         L.xso_update_order.restype = C.c_int
+        L.xso_balanced_order.argtypes = [C.c_uint32, u32p, C.c_uint64, C.c_uint32, C.c_uint32,
+                                         u32p, u32p]
+        L.xso_balanced_order.restype = C.c_int
         L.xso_check_order.argtypes = [C.c_uint32, u32p, u32p, u32p, C.c_uint32]
         L.xso_check_order.restype = C.c_int
         L.xso_init_spins.argtypes = [C.c_uint32, C.c_uint32, C.c_uint64, i8p]
@@ -94,7 +97,7 @@ class Instance:
     """One problem instance: triplets, couplings, adjacency, update order (a-1 of DESIGN.md)."""
 
     def __init__(self, n_spins: int, graph_seed: int, gauge: bool = True, set_cap: int = 0,
-                 tri=None, jbit=None):
+                 tri=None, jbit=None, balanced: bool = False):
         L = lib()
         N = int(n_spins)
         self.N = N
@@ -124,8 +127,19 @@ class Instance:
             raise RuntimeError("not a 3-regular hypergraph")
         self.order = np.zeros(N, dtype=np.uint32)
         ss = np.zeros(N, dtype=np.uint32)
-        self.n_sets = L.xso_update_order(N, _p(self.nbr, C.c_uint32), int(set_cap),
-                                         _p(self.order, C.c_uint32), _p(ss, C.c_uint32))
+        self.n_sets = 0
+        if balanced:
+            # DESIGN.md R-balance: q = max(4, ceil(N / S)) sets, S = set_cap (0 -> 64);
+            # 1000 + 200 N tabu steps; on failure the greedy order below is used
+            S = int(set_cap) if set_cap else 64
+            q = max(4, (N + S - 1) // S)
+            self.n_sets = L.xso_balanced_order(N, _p(self.nbr, C.c_uint32), self.graph_seed, q,
+                                               1000 + 200 * N, _p(self.order, C.c_uint32),
+                                               _p(ss, C.c_uint32))
+        self.balanced = self.n_sets > 0
+        if not self.balanced:
+            self.n_sets = L.xso_update_order(N, _p(self.nbr, C.c_uint32), int(set_cap),
+                                             _p(self.order, C.c_uint32), _p(ss, C.c_uint32))
         if self.n_sets < 0:
             raise RuntimeError("xso_update_order failed")
         self.set_size = ss[: self.n_sets].copy()

@@ -155,7 +155,8 @@ int xs_create_instance(xs_batch** out, const xs_params* p, const uint64_t* graph
         for (uint32_t i = 0; i < p->n_instances; ++i) {
             std::string err;
             if (!build_graph_from_seed(p->n_spins, graph_seeds[i], (p->flags & XS_FLAG_GAUGE) != 0,
-                                       p->set_cap, b->graphs[i], err)) {
+                                       p->set_cap, (p->flags & XS_FLAG_BALANCED) != 0,
+                                       b->graphs[i], err)) {
                 delete b;
                 return fail(XS_EINVAL, err);
             }
@@ -307,7 +308,8 @@ int xs_generate_graph(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uin
     try {
         HostGraph g;
         std::string err;
-        if (!build_graph_from_seed(n_spins, graph_seed, (flags & XS_FLAG_GAUGE) != 0, set_cap, g, err))
+        if (!build_graph_from_seed(n_spins, graph_seed, (flags & XS_FLAG_GAUGE) != 0, set_cap,
+                                   (flags & XS_FLAG_BALANCED) != 0, g, err))
             return fail(XS_EINVAL, err);
         const size_t N = n_spins;
         if (tri) std::memcpy(tri, g.tri.data(), 3 * N * sizeof(uint32_t));

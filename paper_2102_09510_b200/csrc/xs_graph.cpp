@@ -94,10 +94,87 @@ void greedy_sets(HostGraph& g, uint32_t cap)
     }
 }
 
+// Balanced sets (L281: set sizes chosen "to keep the processing of components as balanced as
+// possible"; DESIGN.md R-balance): an equitable colouring with n_col colours found by a tabu
+// search over colour swaps, so that a CTA with `cap` task slots runs ceil(N / cap) full rounds
+// per sweep instead of the greedy partition's 6-7 ragged ones.  All integer, deterministic;
+// random choices come from Philox(ctr = (step, 0, 0, TAG_PARTITION), key = graph seed).
+// Returns false (g.order untouched) if no proper colouring was found within the step budget.
+bool balanced_sets(HostGraph& g, uint64_t seed, uint32_t n_col, uint32_t step_budget)
+{
+    const uint32_t n = g.n;
+    if (n_col < 2 || n_col > n) return false;
+    std::vector<uint32_t> colour(n);
+    std::vector<int32_t> same(static_cast<size_t>(n) * n_col, 0);   // same[v][c]: neighbours of v coloured c
+    std::vector<uint32_t> forbidden_until(static_cast<size_t>(n) * n_col, 0);
+    auto S = [&](uint32_t v, uint32_t c) -> int32_t& { return same[static_cast<size_t>(v) * n_col + c]; };
+    auto F = [&](uint32_t v, uint32_t c) -> uint32_t& { return forbidden_until[static_cast<size_t>(v) * n_col + c]; };
+    for (uint32_t v = 0; v < n; ++v) colour[v] = v % n_col;
+    for (uint32_t v = 0; v < n; ++v)
+        for (int e = 0; e < 6; ++e) ++S(v, colour[g.nbr[6ull * v + e]]);
+    int64_t clashes = 0;      // sum over spins of same-coloured neighbour entries (2 x edges)
+    for (uint32_t v = 0; v < n; ++v) clashes += S(v, colour[v]);
+    int64_t record = clashes;
+    std::vector<uint32_t> clashing;
+    clashing.reserve(n);
+    for (uint32_t step = 1; step <= step_budget && clashes > 0; ++step) {
+        clashing.clear();
+        for (uint32_t v = 0; v < n; ++v)
+            if (S(v, colour[v]) > 0) clashing.push_back(v);
+        uint32_t r[4];
+        rng(step, 0, 0, TAG_PARTITION, seed, r);
+        const uint32_t v = clashing[r[0] % clashing.size()];
+        const uint32_t cv = colour[v];
+        const uint32_t* nv = &g.nbr[6ull * v];
+        int64_t best_gain = 0;
+        uint32_t partner = n;           // n = none yet
+        for (uint32_t u = 0; u < n; ++u) {
+            const uint32_t cu = colour[u];
+            if (cu == cv) continue;
+            const int32_t links = static_cast<int32_t>(std::count(nv, nv + 6, u));
+            const int64_t gain = static_cast<int64_t>(S(v, cu)) - S(v, cv) + S(u, cv) - S(u, cu) - 2 * links;
+            const bool blocked = F(v, cu) >= step || F(u, cv) >= step;
+            if (blocked && clashes + 2 * gain >= record) continue;     // aspiration: a new record
+            if (partner == n || gain < best_gain) { partner = u; best_gain = gain; }
+        }
+        if (partner == n) continue;
+        const uint32_t u = partner, cu = colour[u];
+        for (int e = 0; e < 6; ++e) { const uint32_t w = nv[e]; --S(w, cv); ++S(w, cu); }
+        for (int e = 0; e < 6; ++e) { const uint32_t w = g.nbr[6ull * u + e]; --S(w, cu); ++S(w, cv); }
+        colour[v] = cu;
+        colour[u] = cv;
+        clashes += 2 * best_gain;
+        F(v, cv) = step + 5 + r[1] % 10;
+        F(u, cu) = step + 5 + r[2] % 10;
+        record = std::min(record, clashes);
+    }
+    if (clashes != 0) return false;
+    g.order.clear();
+    g.order.reserve(n);
+    g.set_start.assign(1, 0);
+    for (uint32_t c = 0; c < n_col; ++c) {
+        for (uint32_t v = 0; v < n; ++v)
+            if (colour[v] == c) g.order.push_back(v);
+        g.set_start.push_back(static_cast<uint32_t>(g.order.size()));
+    }
+    return true;
+}
+
+// The update order of a generated instance: balanced on request, else (or on failure) greedy.
+void make_sets(HostGraph& g, uint64_t seed, uint32_t set_cap, bool balanced)
+{
+    if (balanced) {
+        const uint32_t slots = set_cap ? set_cap : 64u;
+        const uint32_t n_col = std::max(4u, (g.n + slots - 1) / slots);
+        if (balanced_sets(g, seed, n_col, 1000u + 200u * g.n)) return;
+    }
+    greedy_sets(g, set_cap);
+}
+
 }  // namespace
 
 bool build_graph_from_seed(uint32_t n, uint64_t graph_seed, bool gauge, uint32_t set_cap,
-                           HostGraph& g, std::string& err)
+                           bool balanced, HostGraph& g, std::string& err)
 {
     g.n = n;
     const uint32_t n_stub = 3u * n;
@@ -139,7 +216,7 @@ bool build_graph_from_seed(uint32_t n, uint64_t graph_seed, bool gauge, uint32_t
             g.jbit[t] = tau[g.tri[3ull * t]] ^ tau[g.tri[3ull * t + 1]] ^ tau[g.tri[3ull * t + 2]];
     }
     if (!derive_adjacency(g, err)) return false;
-    greedy_sets(g, set_cap);
+    make_sets(g, graph_seed, set_cap, balanced);
     return true;
 }
 

@@ -11,7 +11,7 @@
 namespace xs {
 
 // Domain tags in Philox counter word 3.
-enum : uint32_t { TAG_GRAPH = 1, TAG_GAUGE = 2, TAG_INIT = 3, TAG_SWEEP = 4 };
+enum : uint32_t { TAG_GRAPH = 1, TAG_GAUGE = 2, TAG_INIT = 3, TAG_SWEEP = 4, TAG_PARTITION = 5 };
 
 // ---- host-side instance (a-1) -------------------------------------------------------------
 struct HostGraph {
@@ -27,9 +27,9 @@ struct HostGraph {
 
 void philox4x32_10_host(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 
-// Build from seeds (configuration model with rejection, gauge, adjacency, greedy sets).
+// Build from seeds (configuration model with rejection, gauge, adjacency, greedy or balanced sets).
 // Returns false and sets err on failure.
-bool build_graph_from_seed(uint32_t n, uint64_t graph_seed, bool gauge, uint32_t set_cap,
+bool build_graph_from_seed(uint32_t n, uint64_t graph_seed, bool gauge, uint32_t set_cap, bool balanced,
                            HostGraph& g, std::string& err);
 // Build from explicit arrays; validates 3-regularity and that every set is an anti-clique.
 bool build_graph_from_arrays(uint32_t n, const uint32_t* tri, const uint8_t* jbit,

@@ -407,6 +407,7 @@ static cudaError_t launch_one(const StaticArgs& A, uint32_t ctas, uint32_t threa
                               cudaStream_t st, uint32_t rounds)
 {
     // fewer unrolled rounds = fewer registers (the 512-thread variants are capped at 128)
+    if (rounds <= 4) return launch_k<4, CW, NC, MT>(A, ctas, threads, smem, st);
     if (rounds <= 6) return launch_k<6, CW, NC, MT>(A, ctas, threads, smem, st);
     return launch_k<STATIC_MAXT, CW, NC, MT>(A, ctas, threads, smem, st);
 }

@@ -15,8 +15,9 @@ class OracleRun:
     instance was already solved at call entry (and skipping is on)."""
 
     def __init__(self, N, W, graph_seed, run_seed, gauge=True, set_cap=0, thr=W1_THRESHOLD,
-                 no_skip=False, inst: Instance | None = None, words=None, thr4=None):
-        self.inst = inst if inst is not None else Instance(N, graph_seed, gauge, set_cap)
+                 no_skip=False, inst: Instance | None = None, words=None, thr4=None, balanced=False):
+        self.inst = inst if inst is not None else Instance(N, graph_seed, gauge, set_cap,
+                                                           balanced=balanced)
         self.N, self.W, self.run_seed, self.thr, self.no_skip = N, W, run_seed, thr, no_skip
         self.thr4 = thr4                     # general flip table (PAPER.md L67, L69) or None = QG
         # `words`: evolve only this subset of word indices (others stay at their initial value)

@@ -44,6 +44,33 @@ def test_generator_matches_oracle_generator(N, seed, cap, gauge):
     assert o.check_order(order, ss)
 
 
+@pytest.mark.parametrize("N,seed,cap", [(256, 2, 64), (128, 100, 0), (64, 5, 16), (512, 101, 64),
+                                        (20, 3, 0), (100, 4, 32), (6, 1, 0), (3, 1, 0)])
+def test_balanced_sets_match_oracle(N, seed, cap):
+    """XS_FLAG_BALANCED (DESIGN.md R-balance): the library's tabu search and the oracle's are
+    written independently and must produce the same order; it is checked for validity by the
+    oracle (anti-cliques, permutation)."""
+    tri, jbit, order, ss, att = xs.xs_generate_graph(N, seed, xs.XS_FLAG_GAUGE | xs.XS_FLAG_BALANCED, cap)
+    o = Instance(N, seed, gauge=True, set_cap=cap, balanced=True)
+    assert np.array_equal(order, o.order)
+    assert np.array_equal(ss, o.set_size)
+    assert o.check_order(order, ss)
+    # the same two properties straight from the triplets (L277): permutation, and the three spins
+    # of every triplet lie in three different sets
+    assert sorted(order.tolist()) == list(range(N))
+    set_of = np.empty(N, dtype=np.int64)
+    set_of[order] = np.repeat(np.arange(len(ss)), ss)
+    st = set_of[tri.astype(np.int64)]
+    assert (st[:, 0] != st[:, 1]).all() and (st[:, 1] != st[:, 2]).all() and (st[:, 0] != st[:, 2]).all()
+    if o.balanced:
+        S = cap or 64
+        q = max(4, -(-N // S))
+        assert len(ss) == q and int(ss.max()) - int(ss.min()) <= 1 and int(ss.max()) == -(-N // q)
+    else:       # no proper q-colouring found (tiny N): the greedy order
+        g = Instance(N, seed, gauge=True, set_cap=cap)
+        assert np.array_equal(order, g.order)
+
+
 def test_workspace_bytes_and_param_errors():
     p = xs.make_params(256, 1024, 1)
     n = xs.xs_workspace_bytes(p)

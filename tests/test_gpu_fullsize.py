@@ -32,15 +32,20 @@ def _check_words(b, o, inst=0):
         assert np.array_equal(e[sl], eo[sl]), f"energies differ in word {w}"
 
 
-def test_config2_full_size_sampled_words():
-    """configs[1]: N=256, graph seed 2, 2^16 clones; bench.py's geometry (static kernel, T=8)."""
+@pytest.mark.parametrize("balanced", [True, False])
+def test_config2_full_size_sampled_words(balanced):
+    """configs[1]: N=256, graph seed 2, 2^16 clones; bench.py's launch configuration (balanced
+    sets of 64, static kernel, T=8) and the greedy-order variant (`--workload config2_greedy`)."""
     import paper_2102_09510_b200 as xs
     N, W = 256, 1024
-    b = xs.Batch(N, W, [2], [2], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_BALANCED if balanced else 0)
+    b = xs.Batch(N, W, [2], [2], set_cap=64 if balanced else 0, flags=fl)
     lay = b.layout()
     assert (lay.regime, lay.variant, lay.tile_words, lay.ctas) == (0, 1, 8, 128)
+    assert lay.n_sets_max == (4 if balanced else 6)
     words = [0, 7, 8, 517, 1023]          # first/last lane of a tile, tile boundaries, last tile
-    o = OracleRun(N, W, 2, 2, no_skip=True, words=words)
+    o = OracleRun(N, W, 2, 2, set_cap=64 if balanced else 0, no_skip=True, words=words,
+                  balanced=balanced)
     for n in (130, 171):                  # crosses batch boundaries (64) at odd offsets
         b.run_sweeps(n)
         o.run_sweeps(n)

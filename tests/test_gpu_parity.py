@@ -107,6 +107,37 @@ def test_sweep_parity_all_words(N, W, sweeps, tile, variant):
     b.close()
 
 
+@pytest.mark.parametrize("N,W,cap,tile,variant,streaming", [
+    (256, 8, 64, 8, 1, False),     # config-2 tile: 4 full rounds of 64 spins (static kernel, MAXT = 4)
+    (256, 8, 64, 8, 0, False),     # same order on the generic kernel
+    (128, 16, 0, 16, 1, False),    # q = 4 sets of 32
+    (200, 4, 32, 4, 1, False),     # q = 7 sets of 28/29
+    (384, 8, 64, 8, 1, False),     # q = 6
+    (96, 4, 16, 0, 2, True),       # streaming regime
+    (20, 2, 0, 0, 2, False),       # tiny N
+])
+def test_balanced_sets_parity(N, W, cap, tile, variant, streaming):
+    """XS_FLAG_BALANCED (DESIGN.md R-balance): the library builds the balanced order itself (the
+    oracle builds its own); trajectories must agree bit for bit on every kernel."""
+    xs = _xs()
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED
+    if streaming:
+        fl |= xs.XS_FLAG_STREAMING
+    with env(XS_TILE_WORDS=tile, XS_BATCH=16, XS_VARIANT=variant):
+        b = xs.Batch(N, W, [N + 11], [5 * N + 1], set_cap=cap, flags=fl)
+    o = OracleRun(N, W, N + 11, 5 * N + 1, set_cap=cap, no_skip=True, balanced=True)
+    assert o.inst.balanced
+    tri, jbit, order, ss = b.get_graph(0)
+    assert np.array_equal(order, o.inst.order) and np.array_equal(ss, o.inst.set_size)
+    if tile and not streaming:
+        assert b.layout().tile_words == tile and b.layout().variant == variant
+    for n in (17, 1, 30):
+        b.run_sweeps(n)
+        o.run_sweeps(n)
+    _compare(b, [o], f"balanced N={N} W={W}")
+    b.close()
+
+
 @pytest.mark.parametrize("N,W,tile,threads,sweeps", [
     (256, 8, 8, 512, 37),     # config-2 tile, one uint64 word per lane, two row copies
     (100, 16, 16, 512, 23),
