@@ -41,8 +41,12 @@ WORKLOADS = {
                                 "(graph seed 2), 2^16 clones, 10^4 sweeps, no early stop"),
     "config5": dict(N=1 << 20, W=16, I=1, sweeps=100, graph_seed=5, run_seed=5,
                     desc="configs[4]: N=2^20, 1 instance (graph seed 5), 2^10 clones, 100 sweeps (streaming)"),
-    "config3": dict(N=512, W=64, I=256, sweeps=2_000, graph_seed=100, run_seed=100,
-                    desc="configs[2] shape: N=512, 256 instances (seeds 100..355), 2^12 clones each, 2000 sweeps per step"),
+    "config3": dict(N=512, W=64, I=256, sweeps=2_000, graph_seed=100, run_seed=100, balanced=True,
+                    desc="configs[2] shape: N=512, 256 instances (seeds 100..355), 2^12 clones each, 2000 sweeps per step; "
+                         "update order = 4 balanced independent sets of 128"),
+    "config3_greedy": dict(N=512, W=64, I=256, sweeps=2_000, graph_seed=100, run_seed=100,
+                           desc="configs[2] shape with the uncapped greedy sets: N=512, 256 instances (seeds 100..355), "
+                                "2^12 clones each, 2000 sweeps per step"),
     # SURVEY.md F3 / 8(d) "5b": as config 5 with 2^14 clones = 2 GiB of state, DRAM resident
     "config5b": dict(N=1 << 20, W=256, I=1, sweeps=10, graph_seed=5, run_seed=5,
                      desc="config 5b: N=2^20, 1 instance (graph seed 5), 2^14 clones (2 GiB state), 10 sweeps (streaming)"),
@@ -50,13 +54,15 @@ WORKLOADS = {
 # configs[3] shapes: 128 instances (graph seeds 1000 N + i), 2^14 clones each
 for _n, _s in ((128, 2000), (192, 1500), (256, 1000), (384, 700), (512, 500), (768, 350), (1024, 250)):
     WORKLOADS[f"config4_{_n}"] = dict(N=_n, W=256, I=128, sweeps=_s, graph_seed=1000 * _n, run_seed=1000 * _n,
-                                      desc=f"configs[3] shape: N={_n}, 128 instances, 2^14 clones each, {_s} sweeps per step")
+                                      balanced=True,
+                                      desc=f"configs[3] shape: N={_n}, 128 instances, 2^14 clones each, {_s} sweeps "
+                                           f"per step; update order = 4 balanced independent sets")
 ALU_OPS_PER_UPDATE = 14.0 / 32.0      # 14 LOP3/IADD lane-ops per 32 clone-spin updates
 STREAM_BYTES_PER_UPDATE = (8 * 8 * 16 + 28) / 1024.0   # config 5, W=16: 1052 B per 1024 updates
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu
 # --set full captures summarised in profiles/r01_ncu_summary.md (config5: the launch of the
 # largest independent set, 262,053 spin rows = 275.7 MB algorithmic).
-NCU_DRAM_BYTES_PER_LAUNCH = {"config2": 2.43e6, "config2_greedy": 2.43e6, "config3": 91.6e6, "config5": 187.9e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"config2": 2.43e6, "config2_greedy": 2.43e6, "config3": 91.6e6, "config3_greedy": 91.6e6, "config5": 187.9e6}
 
 
 class ClockSampler:

@@ -128,11 +128,10 @@ class Instance:
         self.order = np.zeros(N, dtype=np.uint32)
         ss = np.zeros(N, dtype=np.uint32)
         self.n_sets = 0
-        if balanced:
-            # DESIGN.md R-balance: q = max(4, ceil(N / S)) sets, S = set_cap (0 -> 64);
-            # 1000 + 200 N tabu steps; on failure the greedy order below is used
-            S = int(set_cap) if set_cap else 64
-            q = max(4, (N + S - 1) // S)
+        if balanced and N <= 8192:
+            # DESIGN.md R-balance: q = 4 sets, or max(4, ceil(N / set_cap)) with a set cap;
+            # 1000 + 200 N tabu steps; N > 8192 or a failed search: the greedy order below
+            q = max(4, (N + int(set_cap) - 1) // int(set_cap)) if set_cap else 4
             self.n_sets = L.xso_balanced_order(N, _p(self.nbr, C.c_uint32), self.graph_seed, q,
                                                1000 + 200 * N, _p(self.order, C.c_uint32),
                                                _p(ss, C.c_uint32))

@@ -8,8 +8,10 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libxs_b200.so")
-SOURCES = ["xs_api.cu", "xs_kernels.cu", "xs_sweep_static.cu", "xs_diag.cu", "xs_graph.cpp", "xs_stats.cpp"]
-HEADERS = ["xs_internal.h", "xs_device.cuh", os.path.join("..", "..", "include", "xs.h")]
+OBJ = os.path.join(_HERE, "_obj")      # object cache (git-ignored); sources compile in parallel
+SOURCES = ["xs_api.cu", "xs_kernels.cu", "xs_sweep_static.cu", "xs_diag.cu", "xs_graph.cpp", "xs_stats.cpp"] + \
+          [f"xs_sweep_static_i{cw}{nc}.cu" for cw in (1, 2) for nc in (1, 2, 4)]
+HEADERS = ["xs_internal.h", "xs_device.cuh", "xs_sweep_static.cuh", os.path.join("..", "..", "include", "xs.h")]
 
 
 def _nvcc() -> str:
@@ -30,12 +32,25 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return SO
-    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-           "--shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2",
-           "-o", SO] + [os.path.join(CSRC, s) for s in SOURCES]
+    from concurrent.futures import ThreadPoolExecutor
+    os.makedirs(OBJ, exist_ok=True)
+    nvcc = _nvcc()
+    flags = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+             "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
     if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-    subprocess.check_call(cmd)
+        flags.append("-Xptxas=-v")
+    t_hdr = max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS)
+
+    def compile_one(src: str) -> str:
+        obj = os.path.join(OBJ, src + ".o")
+        path = os.path.join(CSRC, src)
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(t_hdr, os.path.getmtime(path)):
+            subprocess.check_call([nvcc] + flags + ["-c", path, "-o", obj])
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as pool:
+        objs = list(pool.map(compile_one, SOURCES))
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "--shared", "-o", SO] + objs)
     return SO
 
 

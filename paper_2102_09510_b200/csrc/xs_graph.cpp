@@ -96,8 +96,9 @@ void greedy_sets(HostGraph& g, uint32_t cap)
 
 // Balanced sets (L281: set sizes chosen "to keep the processing of components as balanced as
 // possible"; DESIGN.md R-balance): an equitable colouring with n_col colours found by a tabu
-// search over colour swaps, so that a CTA with `cap` task slots runs ceil(N / cap) full rounds
-// per sweep instead of the greedy partition's 6-7 ragged ones.  All integer, deterministic;
+// search over colour swaps: 4 sets (the fewest a graph made of triangles of degree 6 admits in
+// practice) mean 4 barriers per sweep and evenly filled rounds instead of the greedy
+// partition's 6-7 ragged ones; a set cap S asks for max(4, ceil(N / S)) sets.  All integer, deterministic;
 // random choices come from Philox(ctr = (step, 0, 0, TAG_PARTITION), key = graph seed).
 // Returns false (g.order untouched) if no proper colouring was found within the step budget.
 bool balanced_sets(HostGraph& g, uint64_t seed, uint32_t n_col, uint32_t step_budget)
@@ -163,9 +164,8 @@ bool balanced_sets(HostGraph& g, uint64_t seed, uint32_t n_col, uint32_t step_bu
 // The update order of a generated instance: balanced on request, else (or on failure) greedy.
 void make_sets(HostGraph& g, uint64_t seed, uint32_t set_cap, bool balanced)
 {
-    if (balanced) {
-        const uint32_t slots = set_cap ? set_cap : 64u;
-        const uint32_t n_col = std::max(4u, (g.n + slots - 1) / slots);
+    if (balanced && g.n <= 8192u) {     // the search costs O(N) per step: small instances only
+        const uint32_t n_col = set_cap ? std::max(4u, (g.n + set_cap - 1) / set_cap) : 4u;
         if (balanced_sets(g, seed, n_col, 1000u + 200u * g.n)) return;
     }
     greedy_sets(g, set_cap);

@@ -664,6 +664,29 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
                             tile_smem(p.n_spins, 16, 1, b.n_sets_max).total <= SMEM_MAX;
     uint32_t auto_T = 0;
     if (want_variant == 2 && many_tiles && !force_T) auto_T = 16;
+    // Measured: when the update order has few, evenly filled sets
+    // (XS_FLAG_BALANCED: 4 sets of N/4), the static-task kernel on T = 8 tiles with one task per
+    // thread and round (threads = 4 x set size, registers capped so that 16 warps share an SM)
+    // beats the generic kernel also when there are many tiles: 4 barriers per sweep, 8 instead of
+    // 11 shared-memory accesses per task.
+    if (want_variant == 2 && !force_T && !(p.flags & XS_FLAG_STREAMING) && !b.ft.general &&
+        p.n_words % 8 == 0 && (uint64_t)p.n_instances * (p.n_words / 8) >= NUM_SMS) {
+        const uint32_t max_rounds = (p.flags & XS_FLAG_BALANCED) ? 6u : 4u;
+        for (uint32_t lim : {4u, max_rounds}) {
+            for (uint32_t thr : {128u, 256u, 512u}) {
+                if (!static_feasible(b, 8, 2, thr) || static_rounds(b, 8, 2, thr) > lim) continue;
+                g.regime = 0;
+                g.variant = 1;
+                g.T = 8;
+                g.CW = 2;
+                g.threads = thr;
+                g.ctas = p.n_instances * (p.n_words / 8);
+                g.smem = static_smem_bytes(p.n_spins, 8);
+                g.rb = 0;
+                return true;
+            }
+        }
+    }
     // 1) static-task kernel (xs_sweep_static.cu): work list in registers, T in {8,16,32,64}
     // many small tiles (e.g. 20,000 runs of W = 4): the generic kernel's high occupancy wins
     const bool few_tiles = (uint64_t)p.n_instances * ((p.n_words + 7) / 8) < 2ull * NUM_SMS;

@@ -63,8 +63,7 @@ def test_balanced_sets_match_oracle(N, seed, cap):
     st = set_of[tri.astype(np.int64)]
     assert (st[:, 0] != st[:, 1]).all() and (st[:, 1] != st[:, 2]).all() and (st[:, 0] != st[:, 2]).all()
     if o.balanced:
-        S = cap or 64
-        q = max(4, -(-N // S))
+        q = max(4, -(-N // cap)) if cap else 4
         assert len(ss) == q and int(ss.max()) - int(ss.min()) <= 1 and int(ss.max()) == -(-N // q)
     else:       # no proper q-colouring found (tiny N): the greedy order
         g = Instance(N, seed, gauge=True, set_cap=cap)

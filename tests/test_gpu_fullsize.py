@@ -58,23 +58,44 @@ def test_config2_full_size_sampled_words(balanced):
     b.close()
 
 
-def test_config3_shape_sampled_instances_and_words():
-    """configs[2] shape: N=512, W=64 per instance, 160 instances so that every SM gets a tile
-    (generic kernel, T=16 -- the geometry the full 256-instance run uses)."""
+@pytest.mark.parametrize("balanced", [True, False])
+def test_config3_shape_sampled_instances_and_words(balanced):
+    """configs[2] shape: N=512, W=64 per instance, 160 instances so that every SM gets a tile.
+    balanced (bench.py --workload config3): 4 sets of 128 -> static kernel, T=8, 512 threads;
+    greedy (config3_greedy): generic kernel, T=16 -- the geometries the 256-instance runs use."""
     import paper_2102_09510_b200 as xs
     N, W, I = 512, 64, 160
     seeds = list(range(100, 100 + I))
-    b = xs.Batch(N, W, seeds, seeds)
+    b = xs.Batch(N, W, seeds, seeds, flags=xs.XS_FLAG_GAUGE | (xs.XS_FLAG_BALANCED if balanced else 0))
     lay = b.layout()
-    assert (lay.regime, lay.variant, lay.tile_words) == (0, 0, 16)
+    assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == ((0, 1, 8, 512) if balanced else (0, 0, 16, 512))
     checks = {0: [0, 15, 16], 77: [33, 63], 159: [48]}
-    oracles = {i: OracleRun(N, W, seeds[i], seeds[i], words=ws) for i, ws in checks.items()}
+    oracles = {i: OracleRun(N, W, seeds[i], seeds[i], words=ws, balanced=balanced) for i, ws in checks.items()}
     b.run_sweeps(70)
     for i, o in oracles.items():
         o.run_sweeps(70)
         _check_words(b, o, inst=i)
     recs = b.tts()
     assert all(r.sweeps_done == 70 for r in recs)
+    b.close()
+
+
+@pytest.mark.parametrize("N,threads", [(128, 128), (192, 256), (256, 256), (384, 512)])
+def test_config4_shapes_balanced_static_geometry(N, threads):
+    """configs[3] shapes that run on the static kernel in bench.py (--workload config4_N): 160
+    instances of W = 8 give one tile per SM and more; sampled instances, all words."""
+    import paper_2102_09510_b200 as xs
+    W, I = 8, 160
+    seeds = [1000 * N + i for i in range(I)]
+    b = xs.Batch(N, W, seeds, seeds, flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED)
+    lay = b.layout()
+    assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == (0, 1, 8, threads)
+    oracles = {i: OracleRun(N, W, seeds[i], seeds[i], no_skip=True, balanced=True) for i in (0, 101, 159)}
+    for n in (65, 40):
+        b.run_sweeps(n)
+    for i, o in oracles.items():
+        o.run_sweeps(105)
+        _check_words(b, o, inst=i)
     b.close()
 
 
