@@ -286,9 +286,10 @@ def main():
                     "peak_nominal_at_sampled_clock": (148 * 64 * clocks["sm_mhz"] / 1e6) if clocks.get("sm_mhz") else None,
                     "alg_ops_per_update": ALU_OPS_PER_UPDATE, "kernel": "k_sweep_static" if lay.variant == 1 else "k_sweep_tile", "kernel_ms": k_ms}
             # co-limiter: shared-memory pipe, 128 B/clk/SM.  Bytes the kernel's layout
-            # moves per update: static kernel 6 loads + 2 stores of 16 B per 128 updates (T = 8, two
-            # row copies), generic kernel 11 accesses of 16 B per 128 updates.
-            sm_bpu = (8 * 16 / 128.0) if lay.variant == 1 else (11 * 16 / 128.0)
+            # moves per update: static kernel 6 loads + NC stores of 16 B per 128 updates (T = 8: two
+            # row copies, T = 4: four), generic kernel 11 accesses of 16 B per 128 updates.
+            n_copies = 16 // lay.tile_words if lay.tile_words <= 16 else 1            # static kernel: row copies
+            sm_bpu = ((6 + n_copies) * 16 / 128.0) if lay.variant == 1 else (11 * 16 / 128.0)
             if clocks.get("sm_mhz"):
                 sm_peak = 148 * 128 * clocks["sm_mhz"] / 1e3                          # GB/s
                 roof["shared_memory"] = {"bytes_per_update": sm_bpu,

@@ -669,21 +669,24 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     // thread and round (threads = 4 x set size, registers capped so that 16 warps share an SM)
     // beats the generic kernel also when there are many tiles: 4 barriers per sweep, 8 instead of
     // 11 shared-memory accesses per task.
+    // Larger N (sets of more than 128 spins): T = 4 tiles (two lanes per spin, four row copies).
     if (want_variant == 2 && !force_T && !(p.flags & XS_FLAG_STREAMING) && !b.ft.general &&
         p.n_words % 8 == 0 && (uint64_t)p.n_instances * (p.n_words / 8) >= NUM_SMS) {
         const uint32_t max_rounds = (p.flags & XS_FLAG_BALANCED) ? 6u : 4u;
         for (uint32_t lim : {4u, max_rounds}) {
-            for (uint32_t thr : {128u, 256u, 512u}) {
-                if (!static_feasible(b, 8, 2, thr) || static_rounds(b, 8, 2, thr) > lim) continue;
-                g.regime = 0;
-                g.variant = 1;
-                g.T = 8;
-                g.CW = 2;
-                g.threads = thr;
-                g.ctas = p.n_instances * (p.n_words / 8);
-                g.smem = static_smem_bytes(p.n_spins, 8);
-                g.rb = 0;
-                return true;
+            for (uint32_t T : {8u, 4u}) {
+                for (uint32_t thr : {128u, 256u, 512u}) {
+                    if (!static_feasible(b, T, 2, thr) || static_rounds(b, T, 2, thr) > lim) continue;
+                    g.regime = 0;
+                    g.variant = 1;
+                    g.T = T;
+                    g.CW = 2;
+                    g.threads = thr;
+                    g.ctas = p.n_instances * (p.n_words / T);
+                    g.smem = static_smem_bytes(p.n_spins, T);
+                    g.rb = 0;
+                    return true;
+                }
             }
         }
     }

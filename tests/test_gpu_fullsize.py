@@ -80,8 +80,9 @@ def test_config3_shape_sampled_instances_and_words(balanced):
     b.close()
 
 
-@pytest.mark.parametrize("N,threads", [(128, 128), (192, 256), (256, 256), (384, 512)])
-def test_config4_shapes_balanced_static_geometry(N, threads):
+@pytest.mark.parametrize("N,threads,tile", [(128, 128, 8), (192, 256, 8), (256, 256, 8), (384, 512, 8),
+                                            (768, 512, 4)])
+def test_config4_shapes_balanced_static_geometry(N, threads, tile):
     """configs[3] shapes that run on the static kernel in bench.py (--workload config4_N): 160
     instances of W = 8 give one tile per SM and more; sampled instances, all words."""
     import paper_2102_09510_b200 as xs
@@ -89,7 +90,7 @@ def test_config4_shapes_balanced_static_geometry(N, threads):
     seeds = [1000 * N + i for i in range(I)]
     b = xs.Batch(N, W, seeds, seeds, flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED)
     lay = b.layout()
-    assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == (0, 1, 8, threads)
+    assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == (0, 1, tile, threads)
     oracles = {i: OracleRun(N, W, seeds[i], seeds[i], no_skip=True, balanced=True) for i in (0, 101, 159)}
     for n in (65, 40):
         b.run_sweeps(n)
