@@ -60,9 +60,9 @@ for _n, _s in ((128, 2000), (192, 1500), (256, 1000), (384, 700), (512, 500), (7
 ALU_OPS_PER_UPDATE = 14.0 / 32.0      # 14 LOP3/IADD lane-ops per 32 clone-spin updates
 STREAM_BYTES_PER_UPDATE = (8 * 8 * 16 + 28) / 1024.0   # config 5, W=16: 1052 B per 1024 updates
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu
-# --set full captures summarised in profiles/r01_ncu_summary.md (config5: the launch of the
+# --set full captures summarised in profiles/r01_ncu_summary.md and r01b_ncu_summary.md (config5: the launch of the
 # largest independent set, 262,053 spin rows = 275.7 MB algorithmic).
-NCU_DRAM_BYTES_PER_LAUNCH = {"config2": 2.43e6, "config2_greedy": 2.43e6, "config3": 91.6e6, "config3_greedy": 91.6e6, "config5": 187.9e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"config2": 2.42e6, "config2_greedy": 2.43e6, "config3": 93.6e6, "config3_greedy": 91.6e6, "config5": 187.9e6}
 
 
 class ClockSampler:
