@@ -450,6 +450,55 @@ void xso_run_w(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri
     }
 }
 
+/* ---- per-clone noise variant (DESIGN.md R-clone) ------------------
+ * L87: the paper draws ONE random number per word ("the same random number for the 32 clones in
+ * the same word"), which couples the k = 1 decisions of word mates.  This variant gives every
+ * clone its own number: for spin i, word w, sweep t and clone bit b,
+ *     U = sum_{k=0..6} bit_b(r_k) 2^k,   r_{2j} = o0 | o1 << 32,  r_{2j+1} = o2 | o3 << 32
+ *     with (o0..o3) = Philox(ctr = (i, 4w + j, t, 6), key = run seed), j = 0..3  (r_7 unused),
+ * and a spin with k = 1 flips iff U < m, i.e. w1 = m / 128 (m = 7: 0.0547, inside the paper's
+ * 0.054(1), L91).  k >= 2 always flips, k = 0 never (L67).  Same order, same sets as xso_sweep. */
+#define XSO_TAG_CLONE 6u
+void xso_sweep_clone(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint8_t* jbit,
+                     const uint32_t* nbr, const uint32_t* cls, const uint32_t* order,
+                     uint64_t run_seed, uint32_t t, uint32_t m, int8_t* s)
+{
+    for (uint32_t w = w_begin; w < w_end; ++w) {
+        for (uint32_t p = 0; p < N; ++p) {           /* clones are independent: spin outer, clone inner */
+            const uint32_t i = order[p];
+            uint64_t r[8];
+            for (uint32_t j = 0; j < 4u; ++j) {
+                uint32_t o[4];
+                philox_seeded(i, 4u * w + j, t, XSO_TAG_CLONE, run_seed, o);
+                r[2 * j] = (uint64_t)o[0] | ((uint64_t)o[1] << 32);
+                r[2 * j + 1] = (uint64_t)o[2] | ((uint64_t)o[3] << 32);
+            }
+            for (uint32_t b = 0; b < 64u; ++b) {
+                int8_t* s1 = s + ((size_t)64u * w + b) * N;
+                uint32_t U = 0;
+                for (uint32_t k = 0; k < 7u; ++k) U |= (uint32_t)((r[k] >> b) & 1u) << k;
+                const int k_unsat = unsat_count(i, nbr, cls, jbit, s1);
+                const int flip = (k_unsat >= 2) || (k_unsat == 1 && U < m);
+                if (flip) s1[i] = (int8_t)-s1[i];
+            }
+        }
+    }
+}
+
+void xso_run_clone(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri,
+                   const uint8_t* jbit, const uint32_t* nbr, const uint32_t* cls,
+                   const uint32_t* order, uint64_t run_seed, uint32_t t_begin, uint32_t n_sweeps,
+                   uint32_t m, int8_t* s, uint32_t* first_hit)
+{
+    for (uint32_t t = t_begin + 1u; t <= t_begin + n_sweeps; ++t) {
+        xso_sweep_clone(N, w_begin, w_end, jbit, nbr, cls, order, run_seed, t, m, s);
+        for (size_t c = (size_t)64u * w_begin; c < (size_t)64u * w_end; ++c)
+            if (first_hit[c] == 0xFFFFFFFFu &&
+                xso_energy(N, tri, jbit, s + c * N) == -(int32_t)N)
+                first_hit[c] = t;
+    }
+}
+
 void xso_run(uint32_t N, uint32_t w_begin, uint32_t w_end, const uint32_t* tri,
              const uint8_t* jbit, const uint32_t* nbr, const uint32_t* cls,
              const uint32_t* order, const uint32_t* set_size, uint32_t n_sets,

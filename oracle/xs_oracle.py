@@ -70,6 +70,11 @@ def lib():
                                   C.c_int, C.c_int, i8p, u64p, u64p]
         L.xso_run_w.argtypes = [C.c_uint32, C.c_uint32, C.c_uint32, u32p, u8p, u32p, u32p, u32p,
                                 u32p, C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32, u64p, i8p, u32p]
+        # per-clone noise variant
+        L.xso_sweep_clone.argtypes = [C.c_uint32, C.c_uint32, C.c_uint32, u8p, u32p, u32p, u32p,
+                                      C.c_uint64, C.c_uint32, C.c_uint32, i8p]
+        L.xso_run_clone.argtypes = [C.c_uint32, C.c_uint32, C.c_uint32, u32p, u8p, u32p, u32p, u32p,
+                                    C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, i8p, u32p]
         L.xso_pack.argtypes = [C.c_uint32, C.c_uint32, i8p, u64p]
         L.xso_unpack.argtypes = [C.c_uint32, C.c_uint32, u64p, i8p]
         L.xso_omp_threads.restype = C.c_int
@@ -197,13 +202,29 @@ class Instance:
                                _p(self.jbit, C.c_uint8), _p(s, C.c_int8), _p(fh, C.c_uint32))
         return fh
 
+    def sweep_clone(self, s, run_seed, t, m, w_begin=0, w_end=None):
+        """One sweep of the per-clone noise variant (w1 = m / 128), in place."""
+        assert s.dtype == np.int8 and s.flags.c_contiguous
+        w_end = s.shape[0] // 64 if w_end is None else w_end
+        lib().xso_sweep_clone(self.N, w_begin, w_end, _p(self.jbit, C.c_uint8),
+                              _p(self.nbr, C.c_uint32), _p(self.cls, C.c_uint32),
+                              _p(self.order, C.c_uint32), int(run_seed), int(t), int(m),
+                              _p(s, C.c_int8))
+
     def run(self, s, first_hit, run_seed, t_begin, n_sweeps, w_begin=0, w_end=None,
-            thr=W1_THRESHOLD, omp=False, thr4=None):
+            thr=W1_THRESHOLD, omp=False, thr4=None, clone_m=None):
         """Sweeps t_begin+1 .. t_begin+n_sweeps in place, maintaining first_hit."""
         assert s.dtype == np.int8 and s.flags.c_contiguous
         assert first_hit.dtype == np.uint32 and first_hit.flags.c_contiguous
         W = s.shape[0] // 64
         w_end = W if w_end is None else w_end
+        if clone_m is not None:
+            lib().xso_run_clone(self.N, w_begin, w_end, _p(self.tri, C.c_uint32),
+                                _p(self.jbit, C.c_uint8), _p(self.nbr, C.c_uint32),
+                                _p(self.cls, C.c_uint32), _p(self.order, C.c_uint32),
+                                int(run_seed), int(t_begin), int(n_sweeps), int(clone_m),
+                                _p(s, C.c_int8), _p(first_hit, C.c_uint32))
+            return
         if thr4 is not None:
             t4 = np.ascontiguousarray(thr4, dtype=np.uint64)
             lib().xso_run_w(self.N, w_begin, w_end, _p(self.tri, C.c_uint32),

@@ -112,3 +112,20 @@ def sweep(N, W, adj, J, order, run_seed, t, thr, s):
                 k = sum(1 for (c, a, bb) in adj[i] if J[c] * s1[i] * s1[a] * s1[bb] == -1)
                 if k >= 2 or (k == 1 and R):
                     s1[i] = -s1[i]
+
+
+def sweep_clone(N, W, adj, J, order, run_seed, t, m, s):
+    """SURVEY.md 8(f) NEXT-2 (DESIGN.md R-clone): every clone draws its own 7-bit number U from
+    Philox(ctr=(i, 4w+j, t, 6)), j = 0..3; a k = 1 spin flips iff U < m (w1 = m / 128)."""
+    for i in order:
+        for w in range(W):
+            r = []
+            for j in range(4):
+                o = _rng(i, 4 * w + j, t, 6, run_seed)
+                r += [o[0] | (o[1] << 32), o[2] | (o[3] << 32)]
+            for b in range(64):
+                U = sum(((r[k] >> b) & 1) << k for k in range(7))
+                s1 = s[64 * w + b]
+                k = sum(1 for (c, a, bb) in adj[i] if J[c] * s1[i] * s1[a] * s1[bb] == -1)
+                if k >= 2 or (k == 1 and U < m):
+                    s1[i] = -s1[i]
