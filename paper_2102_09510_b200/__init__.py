@@ -7,7 +7,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from ._binding import (XS_FLAG_BALANCED, XS_FLAG_GAUGE, XS_FLAG_NO_SKIP, XS_FLAG_STREAMING,  # noqa: F401
+from ._binding import (XS_FLAG_BALANCED, XS_FLAG_CLONE_NOISE, XS_FLAG_GAUGE, XS_FLAG_NO_SKIP, XS_FLAG_STREAMING,  # noqa: F401
                        XS_NO_HIT,
                        XS_W1_THRESHOLD_DEFAULT, XsError, lib, make_params, xs_alu_peak,
                        xs_create_instance, xs_kernel_launches,

@@ -15,7 +15,7 @@ from . import build as _build
 
 XS_OK, XS_EINVAL, XS_ENOMEM, XS_ECUDA, XS_ESTATE = 0, -1, -2, -3, -4
 XS_NO_HIT = 0xFFFFFFFF
-XS_FLAG_GAUGE, XS_FLAG_NO_SKIP, XS_FLAG_STREAMING, XS_FLAG_BALANCED = 1, 2, 4, 8
+XS_FLAG_GAUGE, XS_FLAG_NO_SKIP, XS_FLAG_STREAMING, XS_FLAG_BALANCED, XS_FLAG_CLONE_NOISE = 1, 2, 4, 8, 16
 XS_W1_THRESHOLD_DEFAULT = 236223201
 
 

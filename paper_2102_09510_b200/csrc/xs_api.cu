@@ -132,7 +132,13 @@ static int finish_create(xs_batch* b, void* dev_ws, size_t ws_bytes, void* strea
     if (cudaError_t e = cudaStreamSynchronize(st)) return cuda_fail((int)e, "upload sync");
 
     // quasi-greedy table (0, w1, 1, 1) of L67 / L101 until xs_set_flip_table says otherwise
-    b->ft = FlipTable{{0u, p.w1_threshold, 0u, 0u}, 0xCu, 0u};
+    b->ft = FlipTable{{0u, p.w1_threshold, 0u, 0u}, 0xCu, 0u, 0u, 0u};
+    if (p.flags & XS_FLAG_CLONE_NOISE) {
+        // per-clone noise: w1 = m / 128 with m the nearest integer; runs in the streaming regime
+        b->ft.per_clone = 1u;
+        b->ft.clone_m = (uint32_t)(((uint64_t)p.w1_threshold + (1ull << 24)) >> 25);
+        b->p.flags |= XS_FLAG_STREAMING;
+    }
     std::string err;
     if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
     if (int e = launch_init(*b, stream)) return cuda_fail(e, "init kernel");
@@ -229,6 +235,13 @@ int xs_set_flip_table(xs_batch* b, const uint64_t* thr4)
     }
     // the quasi-greedy form w = (0, w1 < 1, 1, 1) runs on the fast kernels
     ft.general = !(thr4[0] == 0 && ft.always == 0xCu);
+    if (b->ft.per_clone) {
+        if (thr4[0] != 0 || (ft.always & 0xCu) != 0xCu)
+            return fail(XS_EINVAL, "per-clone noise supports the quasi-greedy form (0, w1, 1, 1) only");
+        ft.general = 0u;
+        ft.per_clone = 1u;
+        ft.clone_m = (uint32_t)((thr4[1] + (1ull << 24)) >> 25);
+    }
     b->ft = ft;
     if (!ft.general) b->p.w1_threshold = ft.lo[1];
     std::string err;

@@ -145,4 +145,19 @@ template <> __device__ __forceinline__ void vstore<2>(void* p, const uint32_t (&
 }
 
 
+// per-clone Bernoulli(m / 128) mask of 32 clones.  r[k] holds bit k of the
+// clones' 7-bit numbers U (bit-sliced); returns the mask of clones with U < m by a most significant
+// bit first comparison against the constant m (m >= 128: all clones).
+__device__ __forceinline__ uint32_t clone_noise_mask(const uint32_t (&r)[7], uint32_t m)
+{
+    if (m >= 128u) return ~0u;
+    uint32_t lt = 0u, eq = ~0u;
+#pragma unroll
+    for (int k = 6; k >= 0; --k) {
+        if ((m >> k) & 1u) { lt |= eq & ~r[k]; eq &= r[k]; }
+        else               { eq &= ~r[k]; }
+    }
+    return lt;
+}
+
 }  // namespace xs

@@ -11,7 +11,7 @@
 namespace xs {
 
 // Domain tags in Philox counter word 3.
-enum : uint32_t { TAG_GRAPH = 1, TAG_GAUGE = 2, TAG_INIT = 3, TAG_SWEEP = 4, TAG_PARTITION = 5 };
+enum : uint32_t { TAG_GRAPH = 1, TAG_GAUGE = 2, TAG_INIT = 3, TAG_SWEEP = 4, TAG_PARTITION = 5, TAG_CLONE = 6 };
 
 // ---- host-side instance (a-1) -------------------------------------------------------------
 struct HostGraph {
@@ -74,6 +74,10 @@ struct FlipTable {
     uint32_t lo[4];
     uint32_t always;
     uint32_t general;
+    // SURVEY.md 8(f) NEXT-2 (XS_FLAG_CLONE_NOISE): every clone draws its own 7-bit number U;
+    // a k = 1 spin flips iff U < clone_m (w1 = clone_m / 128, 0..128)
+    uint32_t per_clone;
+    uint32_t clone_m;
 };
 
 struct TileGeom {

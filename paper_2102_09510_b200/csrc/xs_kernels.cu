@@ -495,7 +495,8 @@ __device__ __forceinline__ void pdl_wait_and_release()
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
-template <int CW>
+// PC: per-clone noise instead of one number per word.
+template <int CW, bool PC>
 __global__ void __launch_bounds__(ST_THREADS) k_stream_set(DevPtrs d, uint32_t N, uint32_t W,
                                                           uint32_t set_idx, uint32_t s_rel,
                                                           FlipTable ft, uint32_t flags, uint64_t* det)
@@ -547,15 +548,36 @@ __global__ void __launch_bounds__(ST_THREADS) k_stream_set(DevPtrs d, uint32_t N
         const uint32_t jm0 = (r1.w & 1u) ? ~0u : 0u, jm1 = (r1.w & 2u) ? ~0u : 0u,
                        jm2 = (r1.w & 4u) ? ~0u : 0u;
         uint32_t o[4];
-        philox4x32_10(r1.z, w >> 2, t, TAG_SWEEP, k0, k1, o);
+        if (!PC) philox4x32_10(r1.z, w >> 2, t, TAG_SWEEP, k0, k1, o);
         uint32_t xn[2 * CW];
+        uint32_t Rc[2 * CW];       // PC: k = 1 flip masks of the lane's half words
+        if (PC) {
+#pragma unroll
+            for (int c = 0; c < CW; ++c) {
+                uint32_t rl[8], rh[8];   // low / high halves of r_0 .. r_7 of word w + c
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    uint32_t q4[4];
+                    philox4x32_10(r1.z, 4u * (w + c) + jj, t, TAG_CLONE, k0, k1, q4);
+                    rl[2 * jj] = q4[0]; rh[2 * jj] = q4[1];
+                    rl[2 * jj + 1] = q4[2]; rh[2 * jj + 1] = q4[3];
+                }
+                const uint32_t lo7[7] = {rl[0], rl[1], rl[2], rl[3], rl[4], rl[5], rl[6]};
+                const uint32_t hi7[7] = {rh[0], rh[1], rh[2], rh[3], rh[4], rh[5], rh[6]};
+                Rc[2 * c] = clone_noise_mask(lo7, ft.clone_m);
+                Rc[2 * c + 1] = clone_noise_mask(hi7, ft.clone_m);
+            }
+        }
 #pragma unroll
         for (int h = 0; h < 2 * CW; ++h) {
-            const uint32_t u = (((w + (h >> 1)) & 3u) == 0u) ? o[0] : (((w + (h >> 1)) & 3u) == 1u) ? o[1]
+            const uint32_t u = PC ? 0u : (((w + (h >> 1)) & 3u) == 0u) ? o[0] : (((w + (h >> 1)) & 3u) == 1u) ? o[1]
                                : (((w + (h >> 1)) & 3u) == 2u) ? o[2] : o[3];
             const uint32_t nz = qg_nonzero_k(a[0][h], b[0][h], jm0, a[1][h], b[1][h], jm1, a[2][h],
                                              b[2][h], jm2, xo[h]);
-            if (ft.general) {
+            if (PC) {
+                xn[h] = qg_update(a[0][h], b[0][h], jm0, a[1][h], b[1][h], jm1, a[2][h], b[2][h], jm2,
+                                  xo[h], Rc[h]);
+            } else if (ft.general) {
                 uint32_t Rk[4];
 #pragma unroll
                 for (int k = 0; k < 4; ++k)
@@ -902,12 +924,9 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
             cfg.stream = st;
             cfg.attrs = pdl_attr;
             cfg.numAttrs = 1;
-            if (g.CW == 2)
-                XS_CU(cudaLaunchKernelEx(&cfg, k_stream_set<2>, b.d, p.n_spins, p.n_words, set, s, b.ft,
-                                         p.flags, cur));
-            else
-                XS_CU(cudaLaunchKernelEx(&cfg, k_stream_set<1>, b.d, p.n_spins, p.n_words, set, s, b.ft,
-                                         p.flags, cur));
+            auto kern = b.ft.per_clone ? (g.CW == 2 ? k_stream_set<2, true> : k_stream_set<1, true>)
+                                       : (g.CW == 2 ? k_stream_set<2, false> : k_stream_set<1, false>);
+            XS_CU(cudaLaunchKernelEx(&cfg, kern, b.d, p.n_spins, p.n_words, set, s, b.ft, p.flags, cur));
             count_launch(1);
         }
         if (b.ft.lo[0] != 0u || (b.ft.always & 1u)) {

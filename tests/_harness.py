@@ -15,11 +15,13 @@ class OracleRun:
     instance was already solved at call entry (and skipping is on)."""
 
     def __init__(self, N, W, graph_seed, run_seed, gauge=True, set_cap=0, thr=W1_THRESHOLD,
-                 no_skip=False, inst: Instance | None = None, words=None, thr4=None, balanced=False):
+                 no_skip=False, inst: Instance | None = None, words=None, thr4=None, balanced=False,
+                 clone_m=None):
         self.inst = inst if inst is not None else Instance(N, graph_seed, gauge, set_cap,
                                                            balanced=balanced)
         self.N, self.W, self.run_seed, self.thr, self.no_skip = N, W, run_seed, thr, no_skip
         self.thr4 = thr4                     # general flip table (PAPER.md L67, L69) or None = QG
+        self.clone_m = clone_m               # per-clone noise variant (NEXT-2): w1 = clone_m / 128
         # `words`: evolve only this subset of word indices (others stay at their initial value)
         self.words = list(range(W)) if words is None else sorted(words)
         self.s = self.inst.init_spins(W, run_seed)
@@ -39,7 +41,7 @@ class OracleRun:
             return
         for w in self.words:
             self.inst.run(self.s, self.first_hit, self.run_seed, self.sweeps_done, n, w, w + 1,
-                          thr=self.thr, thr4=self.thr4)
+                          thr=self.thr, thr4=self.thr4, clone_m=self.clone_m)
         self.sweeps_done += n
 
     def x(self) -> np.ndarray:
