@@ -50,6 +50,10 @@ WORKLOADS = {
     # SURVEY.md F3 / 8(d) "5b": as config 5 with 2^14 clones = 2 GiB of state, DRAM resident
     "config5b": dict(N=1 << 20, W=256, I=1, sweeps=10, graph_seed=5, run_seed=5,
                      desc="config 5b: N=2^20, 1 instance (graph seed 5), 2^14 clones (2 GiB state), 10 sweeps (streaming)"),
+    # config 5 with an independent random number per clone (16 x the Philox work)
+    "config5_clone_noise": dict(N=1 << 20, W=16, I=1, sweeps=20, graph_seed=5, run_seed=5, clone_noise=True,
+                                desc="configs[4] with per-clone noise (XS_FLAG_CLONE_NOISE, w1 = 7/128): N=2^20, 1 instance "
+                                     "(graph seed 5), 2^10 clones, 20 sweeps (streaming)"),
 }
 # configs[3] shapes: 128 instances (graph seeds 1000 N + i), 2^14 clones each
 for _n, _s in ((128, 2000), (192, 1500), (256, 1000), (384, 700), (512, 500), (768, 350), (1024, 250)):
@@ -115,15 +119,18 @@ def cpu_oracle_rate(wl, target_s: float = 20.0):
     cores = omp_threads()
     N = wl["N"]
     inst = Instance(N, wl["graph_seed"], True, wl.get("set_cap", 0), balanced=bool(wl.get("balanced")))
+    clone_m = 7 if wl.get("clone_noise") else None          # the variant's oracle is single threaded
+    if clone_m is not None:
+        cores = 1
     W = max(1, min(wl["W"], 4 * cores))      # enough words for ~target_s of work on all cores
     s = inst.init_spins(W, wl["run_seed"])
     fh = np.full(64 * W, NO_HIT, np.uint32)
     t0 = time.perf_counter()
-    inst.run(s, fh, wl["run_seed"], 0, 1, omp=True)         # calibration sweep
+    inst.run(s, fh, wl["run_seed"], 0, 1, omp=True, clone_m=clone_m)         # calibration sweep
     dt1 = max(time.perf_counter() - t0, 1e-6)
     sweeps = int(max(1, min(wl["sweeps"], target_s / dt1)))
     t0 = time.perf_counter()
-    inst.run(s, fh, wl["run_seed"], 1, sweeps, omp=True)
+    inst.run(s, fh, wl["run_seed"], 1, sweeps, omp=True, clone_m=clone_m)
     dt = time.perf_counter() - t0
     rate = N * 64.0 * W * sweeps / (dt * 1e9)
     return {"value": rate, "unit": "clone-spin updates/ns", "cores": cores, "kind": "oracle",
@@ -187,7 +194,8 @@ def main():
     gseeds = [wl["graph_seed"] + i for i in range(I)]
     from paper_2102_09510_b200 import replicas
     rseeds = replicas.replica_run_seeds([wl["run_seed"] + i for i in range(I)], rank)   # replicas (L87)
-    flags = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_BALANCED if wl.get("balanced") else 0)
+    flags = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_BALANCED if wl.get("balanced") else 0) | \
+        (xs.XS_FLAG_CLONE_NOISE if wl.get("clone_noise") else 0)
     b = xs.Batch(N, W, gseeds, rseeds, set_cap=wl.get("set_cap", 0), flags=flags, device=dev)
     lay = b.layout()
     updates_per_step = float(N) * 64.0 * W * I * sweeps

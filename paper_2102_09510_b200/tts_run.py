@@ -119,13 +119,24 @@ def main():
     ap.add_argument("--cap", type=int, default=200000)
     ap.add_argument("--chunk", type=int, default=100)
     ap.add_argument("--seed0", type=int, default=100)
+    ap.add_argument("--balanced", action="store_true",
+                    help="update order = 4 balanced independent sets (XS_FLAG_BALANCED) instead of the greedy sets")
+    ap.add_argument("--clone-noise", action="store_true",
+                    help="SURVEY.md 8(f) NEXT-2: an independent random number per clone (w1 = m/128, m = round(128 w1)) "
+                         "instead of one per word (PAPER.md L87)")
     ap.add_argument("--w1", type=float, nargs="*", default=None,
                     help="scan of w1 (PAPER.md Fig. 1, L91/L101: optimum 0.054(1)); default 0.055")
     args = ap.parse_args()
     rows = []
     for n in args.n:
         for w1 in (args.w1 or [None]):
-            r = run_size(n, args.words, args.instances, args.runs, args.cap, args.chunk, args.seed0, w1=w1)
+            import paper_2102_09510_b200 as xs
+            fx = (xs.XS_FLAG_BALANCED if args.balanced else 0) | (xs.XS_FLAG_CLONE_NOISE if args.clone_noise else 0)
+            r = run_size(n, args.words, args.instances, args.runs, args.cap, args.chunk, args.seed0,
+                         flags_extra=fx, w1=w1)
+            r["update_order"] = "balanced" if args.balanced else "greedy"
+            r["noise"] = "per clone" if args.clone_noise else "per word"
+
             rows.append(r)
             print(json.dumps(r), flush=True)
     if args.w1:
