@@ -186,6 +186,20 @@ int xs_get_layout(const xs_batch* b, xs_layout* out);
  *               scale T_tot) (L145); for n = 0, out[9] = T_tot / ln 20 (95 % lower bound), rest inf. */
 int xs_tts_stats(const uint32_t* tts, uint32_t n_runs, uint64_t t_max, double* out /* [12] */);
 
+/* SURVEY.md 8(f) NEXT-4.  Cavity prediction of the growth rate of the time to solution
+ * (Eqs. (3)-(4)): K-spin model on a K-regular random hypergraph at temperature
+ * T with a field b that sets the magnetisation m.  With tanh(beta u) = tanh(beta) tanh(beta h)^(K-1),
+ * b = h - (K-1) u, m = tanh(beta (u + h)) (Eq. (4)) the free energy along the one-parameter family h is
+ *   -beta f = log Z_i + log Z_a - K log Z_ai - beta b m          (Eq. (3); DESIGN.md R-eq3),
+ * f_para = -log(2 cosh beta) / beta.  Host only, double precision.
+ *   out[0] = beta max_m (f - f_para)  (the barrier; 0.0827249 at K = 3, T_run = -2/ln 0.055, L208)
+ *   out[1] = m at the barrier          out[2] = h at the barrier
+ *   out[3] = T_sp(K), 1/T_sp = min_x atanh[tanh(x) / tanh((K-1)x)^(K-1)]  (0.980548 for K = 3, L198)
+ *   out[4] = beta (f - f_para) of the ferromagnetic state (b = 0, m > 0), out[5] = its m.
+ * T >= T_sp: no ferromagnetic solution, out[0..2] and out[4..5] are NaN (out[3] is still set).
+ * Returns XS_EINVAL for K < 3 or T <= 0. */
+int xs_cavity_barrier(uint32_t K, double T, double* out /* [6] */);
+
 /* Measurement helpers (no arithmetic of the method).
  * xs_alu_peak: runs a pure-LOP3 micro-kernel (16 independent chains per thread, all SMs) and
  *   returns the measured integer-pipe rate in 32-bit lane-operations per nanosecond for the

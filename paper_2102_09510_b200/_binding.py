@@ -38,7 +38,7 @@ class xs_layout(C.Structure):
 EXPORTS = ["xs_workspace_bytes", "xs_create_instance", "xs_create_instance_from_arrays",
            "xs_run_sweeps", "xs_set_flip_table", "xs_energy", "xs_tts", "xs_get_spins", "xs_set_spins",
            "xs_get_first_hit", "xs_get_graph", "xs_generate_graph", "xs_get_layout", "xs_tts_stats",
-           "xs_alu_peak", "xs_kernel_launches", "xs_destroy",
+           "xs_cavity_barrier", "xs_alu_peak", "xs_kernel_launches", "xs_destroy",
            "xs_last_error"]
 
 _lib = None
@@ -71,6 +71,7 @@ def lib():
                                     u32p, u32p, C.POINTER(C.c_int32)]
     L.xs_get_layout.argtypes = [vp, C.POINTER(xs_layout)]
     L.xs_tts_stats.argtypes = [u32p, C.c_uint32, C.c_uint64, C.POINTER(C.c_double)]
+    L.xs_cavity_barrier.argtypes = [C.c_uint32, C.c_double, C.POINTER(C.c_double)]
     L.xs_destroy.argtypes = [vp]
     L.xs_alu_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
     L.xs_kernel_launches.argtypes = []
@@ -222,6 +223,14 @@ def xs_tts_stats(tts, t_max: int) -> dict:
     _check(lib().xs_tts_stats(_ptr(t, C.c_uint32), t.size, int(t_max), out), "xs_tts_stats")
     keys = ["n_solved", "t_tot", "tau_hat", "tts50_model", "tts90_model", "tts99_model",
             "tts50_emp", "tts90_emp", "tts99_emp", "tau_q16", "tau_q50", "tau_q84"]
+    return dict(zip(keys, [float(v) for v in out]))
+
+
+def xs_cavity_barrier(K: int, T: float) -> dict:
+    """PAPER.md Eqs. (3)-(4): cavity free-energy barrier of the K-spin model at temperature T."""
+    out = (C.c_double * 6)()
+    _check(lib().xs_cavity_barrier(int(K), float(T), out), "xs_cavity_barrier")
+    keys = ["barrier", "m_barrier", "h_barrier", "T_sp", "ferro_bdf", "m_ferro"]
     return dict(zip(keys, [float(v) for v in out]))
 
 
