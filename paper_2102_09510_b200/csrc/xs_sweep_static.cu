@@ -75,6 +75,19 @@ int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream)
     L.rounds = static_rounds(b, g.T, g.CW, g.threads);
     L.threads = g.threads; L.ctas = g.ctas; L.smem = g.smem;
     L.dense = g.ctas > 148u;
+    // FULL: exactly `rounds` sets, one round each, and the last warp of the CTA has a task in each
+    {
+        const uint32_t n_slots = g.threads / (g.T / g.CW), slots_per_warp = 32u / (g.T / g.CW);
+        const uint32_t warps = g.threads / 32u;
+        L.full = slots_per_warp > 0;
+        for (const HostGraph& hg : b.graphs) {
+            if (hg.set_start.size() != (size_t)L.rounds + 1) { L.full = false; break; }
+            for (size_t s = 0; s + 1 < hg.set_start.size(); ++s) {
+                const uint32_t sz = hg.set_start[s + 1] - hg.set_start[s];
+                if (sz > n_slots || sz <= (warps - 1) * slots_per_warp) L.full = false;
+            }
+        }
+    }
     L.st = (cudaStream_t)stream;
     cudaError_t e;
     if (g.CW == 2)

@@ -87,7 +87,9 @@ struct Tasks {
 
 // MAXT: unrolled rounds per sweep; MAXTHREADS / MINB: launch bounds (MINB > 1 caps the registers so
 // that several CTAs share an SM when there are more tiles than SMs).
-template <int MAXT, int CW, int NC, int MAXTHREADS, int MINB>
+// FULL: every instance has exactly MAXT sets of one round each and every warp has a task in every
+// round (balanced sets on a matching CTA size): the round loop carries no tests at all.
+template <int MAXT, int CW, int NC, int MAXTHREADS, int MINB, bool FULL>
 __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_static(StaticArgs A)
 {
     constexpr int H = 2 * CW;          // uint32 halves per lane
@@ -227,8 +229,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_static(StaticArgs A)
         constexpr uint32_t sel0 = 0x8888u + 0x1111u * (CW * h);
 #pragma unroll
         for (int r = 0; r < MAXT; ++r) {
-            if (r < (int)tk.n_rounds) {
-                if ((tk.wact >> r) & 1u) {
+            if (FULL || r < (int)tk.n_rounds) {
+                if (FULL || ((tk.wact >> r) & 1u)) {
                     uint32_t a0[H], b0[H], a1[H], b1[H], a2[H], b2[H], xn[H];
                     lds<CW>(tk.a[r][0], a0); lds<CW>(tk.a[r][1], b0);
                     lds<CW>(tk.a[r][2], a1); lds<CW>(tk.a[r][3], b1);
@@ -249,7 +251,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_static(StaticArgs A)
 #pragma unroll
                     for (int c = 0; c < H; ++c) tk.x[r][c] = xn[c];
                 }
-                if ((tk.bar >> r) & 1u) __syncthreads();
+                if (FULL || ((tk.bar >> r) & 1u)) __syncthreads();
             }
         }
     };
@@ -353,16 +355,17 @@ struct StaticLaunch {
     uint32_t rounds;     // rounds per sweep (<= 8)
     uint32_t threads, ctas, smem;
     bool dense;          // more CTAs than SMs: prefer the register-capped variants
+    bool full;           // see FULL
     cudaStream_t st;
 };
 
-template <int MAXT, int CW, int NC, int MT, int MINB>
+template <int MAXT, int CW, int NC, int MT, int MINB, bool FULL>
 cudaError_t launch_static_k(const StaticArgs& A, const StaticLaunch& L)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_static<MAXT, CW, NC, MT, MINB>,
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_static<MAXT, CW, NC, MT, MINB, FULL>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem);
     if (e != cudaSuccess) return e;
-    k_sweep_static<MAXT, CW, NC, MT, MINB><<<L.ctas, L.threads, L.smem, L.st>>>(A);
+    k_sweep_static<MAXT, CW, NC, MT, MINB, FULL><<<L.ctas, L.threads, L.smem, L.st>>>(A);
     return cudaGetLastError();
 }
 
@@ -370,9 +373,10 @@ template <int CW, int NC, int MT, int MINB>
 cudaError_t launch_static_t(const StaticArgs& A, const StaticLaunch& L)
 {
     // fewer unrolled rounds = fewer registers
-    if (L.rounds <= 4) return launch_static_k<4, CW, NC, MT, MINB>(A, L);
-    if (L.rounds <= 6) return launch_static_k<6, CW, NC, MT, MINB>(A, L);
-    return launch_static_k<8, CW, NC, MT, MINB>(A, L);
+    if (L.rounds == 4 && L.full) return launch_static_k<4, CW, NC, MT, MINB, true>(A, L);
+    if (L.rounds <= 4) return launch_static_k<4, CW, NC, MT, MINB, false>(A, L);
+    if (L.rounds <= 6) return launch_static_k<6, CW, NC, MT, MINB, false>(A, L);
+    return launch_static_k<8, CW, NC, MT, MINB, false>(A, L);
 }
 
 template <int CW, int NC>
