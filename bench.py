@@ -60,7 +60,7 @@ for _n, _s in ((128, 2000), (192, 1500), (256, 1000), (384, 700), (512, 500), (7
     WORKLOADS[f"config4_{_n}"] = dict(N=_n, W=256, I=128, sweeps=_s, graph_seed=1000 * _n, run_seed=1000 * _n,
                                       balanced=True,
                                       desc=f"configs[3] shape: N={_n}, 128 instances, 2^14 clones each, {_s} sweeps "
-                                           f"per step; update order = 4 balanced independent sets")
+                                           f"per step; update order = balanced independent sets (DESIGN.md R-balance)")
 ALU_OPS_PER_UPDATE = 14.0 / 32.0      # 14 LOP3/IADD lane-ops per 32 clone-spin updates
 STREAM_BYTES_PER_UPDATE = (8 * 8 * 16 + 28) / 1024.0   # config 5, W=16: 1052 B per 1024 updates
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu

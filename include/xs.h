@@ -55,8 +55,9 @@ extern "C" {
                                     on chip; the regimes are bit-identical (tests use this)             */
 #define XS_FLAG_BALANCED     8u  /* generated instances: balanced independent sets instead of the
                                     greedy ones (L281: sets sized to keep the lanes evenly busy).
-                                    q = 4 sets of equal size (within one), or max(4, ceil(N/set_cap))
-                                    with a set cap, found by a deterministic tabu search seeded by
+                                    q = max(4, ceil(N/S)) sets of equal size (within one), S = set_cap
+                                    or by default the largest of 16..256 (powers of two) <= N/4,
+                                    found by a deterministic tabu search seeded by
                                     the graph seed (DESIGN.md R-balance); N > 8192 or a failed search:
                                     the greedy sets.  A different, equally valid update order:
                                     trajectories differ from the greedy order's                         */

@@ -134,9 +134,15 @@ class Instance:
         ss = np.zeros(N, dtype=np.uint32)
         self.n_sets = 0
         if balanced and N <= 8192:
-            # DESIGN.md R-balance: q = 4 sets, or max(4, ceil(N / set_cap)) with a set cap;
+            # DESIGN.md R-balance: q = max(4, ceil(N / S)) sets, S = set_cap or, by default, the
+            # largest of 16, 32, 64, 128, 256 with S <= N / 4 (16 if there is none);
             # 1000 + 200 N tabu steps; N > 8192 or a failed search: the greedy order below
-            q = max(4, (N + int(set_cap) - 1) // int(set_cap)) if set_cap else 4
+            S = int(set_cap)
+            if S == 0:
+                S = 16
+                while S < 256 and 2 * S <= N // 4:
+                    S *= 2
+            q = max(4, (N + S - 1) // S)
             self.n_sets = L.xso_balanced_order(N, _p(self.nbr, C.c_uint32), self.graph_seed, q,
                                                1000 + 200 * N, _p(self.order, C.c_uint32),
                                                _p(ss, C.c_uint32))

@@ -96,9 +96,9 @@ void greedy_sets(HostGraph& g, uint32_t cap)
 
 // Balanced sets (L281: set sizes chosen "to keep the processing of components as balanced as
 // possible"; DESIGN.md R-balance): an equitable colouring with n_col colours found by a tabu
-// search over colour swaps: 4 sets (the fewest a graph made of triangles of degree 6 admits in
-// practice) mean 4 barriers per sweep and evenly filled rounds instead of the greedy
-// partition's 6-7 ragged ones; a set cap S asks for max(4, ceil(N / S)) sets.  All integer, deterministic;
+// search over colour swaps into max(4, ceil(N / S)) sets, S = the set cap or a power of two near
+// N / 4: few barriers per sweep and evenly filled rounds instead of the greedy partition's 6-7
+// ragged ones (4 colours are the fewest a graph made of triangles of degree 6 admits in practice).  All integer, deterministic;
 // random choices come from Philox(ctr = (step, 0, 0, TAG_PARTITION), key = graph seed).
 // Returns false (g.order untouched) if no proper colouring was found within the step budget.
 bool balanced_sets(HostGraph& g, uint64_t seed, uint32_t n_col, uint32_t step_budget)
@@ -165,7 +165,15 @@ bool balanced_sets(HostGraph& g, uint64_t seed, uint32_t n_col, uint32_t step_bu
 void make_sets(HostGraph& g, uint64_t seed, uint32_t set_cap, bool balanced)
 {
     if (balanced && g.n <= 8192u) {     // the search costs O(N) per step: small instances only
-        const uint32_t n_col = set_cap ? std::max(4u, (g.n + set_cap - 1) / set_cap) : 4u;
+        // default set size: the largest of 16, 32, 64, 128, 256 that still leaves at least 4 sets
+        // (N = 256 -> 4 x 64, N = 192 -> 6 x 32, N = 512 -> 4 x 128): sets that fill a CTA of
+        // 4 x size threads exactly
+        uint32_t size = set_cap;
+        if (size == 0) {
+            size = 16;
+            while (size < 256 && 2 * size <= g.n / 4) size *= 2;
+        }
+        const uint32_t n_col = std::max(4u, (g.n + size - 1) / size);
         if (balanced_sets(g, seed, n_col, 1000u + 200u * g.n)) return;
     }
     greedy_sets(g, set_cap);

@@ -45,7 +45,8 @@ def test_generator_matches_oracle_generator(N, seed, cap, gauge):
 
 
 @pytest.mark.parametrize("N,seed,cap", [(256, 2, 64), (128, 100, 0), (64, 5, 16), (512, 101, 64),
-                                        (20, 3, 0), (100, 4, 32), (6, 1, 0), (3, 1, 0)])
+                                        (20, 3, 0), (100, 4, 32), (6, 1, 0), (3, 1, 0), (192, 7, 0), (384, 8, 0),
+                                        (768, 9, 0), (1024, 10, 0), (320, 11, 0)])
 def test_balanced_sets_match_oracle(N, seed, cap):
     """XS_FLAG_BALANCED (DESIGN.md R-balance): the library's tabu search and the oracle's are
     written independently and must produce the same order; it is checked for validity by the
@@ -63,7 +64,10 @@ def test_balanced_sets_match_oracle(N, seed, cap):
     st = set_of[tri.astype(np.int64)]
     assert (st[:, 0] != st[:, 1]).all() and (st[:, 1] != st[:, 2]).all() and (st[:, 0] != st[:, 2]).all()
     if o.balanced:
-        q = max(4, -(-N // cap)) if cap else 4
+        S = cap
+        if S == 0:                                   # default: largest power of two in 16..256 below N/4
+            S = max([v for v in (16, 32, 64, 128, 256) if v <= N // 4] or [16])
+        q = max(4, -(-N // S))
         assert len(ss) == q and int(ss.max()) - int(ss.min()) <= 1 and int(ss.max()) == -(-N // q)
     else:       # no proper q-colouring found (tiny N): the greedy order
         g = Instance(N, seed, gauge=True, set_cap=cap)
