@@ -1,6 +1,6 @@
 // xs_sweep_static.cuh -- the static-task sweep kernel (template).  Included by the instantiation
-// units xs_sweep_static_i*.cu (one per (CW, NC), so that they compile in parallel) and by nothing else.
-//
+// units xs_sweep_static_i*.cu (one per (CW, NC), so that they compile in parallel) and by the host
+// side xs_sweep_static.cu (declarations only).
 //
 // Same tile ownership as k_sweep_tile (a CTA keeps (instance, T word columns) in shared
 // memory for the whole call; lanes <-> clone words of one spin row, sets
