@@ -304,3 +304,38 @@ def test_error_codes_on_gpu():
     with pytest.raises(xs.XsError) as ei:
         xs.xs_create_instance(p, [1], [1], ws.data_ptr() // 256 * 256 + 256, 16)
     assert ei.value.code == -2
+
+
+@pytest.mark.parametrize("case", range(16))
+def test_random_shapes_and_flags_parity(case):
+    """Seeded random (N, W, instances, order, regime) combinations through whatever geometry the
+    library picks (no overrides): the geometry rule must never change results."""
+    xs = _xs()
+    rng = np.random.default_rng(1000 + case)
+    N = int(rng.choice([12, 24, 48, 64, 100, 128, 160, 192, 256, 320, 384]))
+    W = int(rng.choice([1, 2, 4, 8, 8, 16, 24]))
+    I = int(rng.choice([1, 3, 40, 160])) if N <= 256 and W <= 8 else int(rng.choice([1, 2]))
+    balanced = bool(rng.integers(0, 2))
+    cap = int(rng.choice([0, 0, 16, 32, 64]))
+    streaming = bool(rng.integers(0, 4) == 0)
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_BALANCED if balanced else 0) | \
+        (xs.XS_FLAG_STREAMING if streaming else 0)
+    gseeds = [5000 + 17 * case + i for i in range(I)]
+    rseeds = [9000 + 31 * case + i for i in range(I)]
+    b = xs.Batch(N, W, gseeds, rseeds, set_cap=cap, flags=fl)
+    lay = b.layout()
+    check = sorted(set([0, I - 1, I // 2]))
+    oracles = {i: OracleRun(N, W, gseeds[i], rseeds[i], set_cap=cap, no_skip=True, balanced=balanced)
+               for i in check}
+    for n in (int(rng.integers(1, 40)), int(rng.integers(1, 80))):
+        b.run_sweeps(n)
+        for o in oracles.values():
+            o.run_sweeps(n)
+    x, fh, e = b.spins_numpy(), b.first_hit_numpy(), b.energy().cpu().numpy()
+    for i, o in oracles.items():
+        what = f"case {case}: N={N} W={W} I={I} bal={balanced} cap={cap} stream={streaming} " \
+               f"regime={lay.regime} variant={lay.variant} T={lay.tile_words} thr={lay.threads} inst={i}"
+        assert np.array_equal(x[i], o.x()), what
+        assert np.array_equal(fh[i], o.first_hit), what
+        assert np.array_equal(e[i], o.energy()), what
+    b.close()
