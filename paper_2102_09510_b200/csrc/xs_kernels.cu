@@ -4,7 +4,10 @@
 //   k_init          a-2   random initial clone words from Philox(INIT)
 //   k_sweep_tile    a-3..a-10  on-chip regime: a CTA owns (instance, T word columns), keeps the
 //                   tile in shared memory for all sweeps of the call               (L293-L295)
-//   k_stream_set    a-4..a-9   streaming regime: one launch per independent set, state in HBM/L2
+//   k_stream_set    a-4..a-9   streaming regime: one launch per independent set, state in HBM/L2;
+//                   <CW, true>: per-clone noise variant
+//   (k_sweep_static, the register-resident work-list kernel of configs 2-4, lives in
+//    xs_sweep_static.cuh)
 //   k_unsat_or / k_mark / k_stream_commit   a-9/a-11  ground-state detection, first-hit table
 //   k_energy_*      a-11  per-clone energies                                       (L41 Eq.(1))
 //   k_finalize      a-11/a-12  per-instance min first-hit, solved flag, sweep counter (L111)
