@@ -113,6 +113,16 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def energy_histogram(e):
+    """Final energy histogram over all clones (north_star: configs[1] reports it): [[E, count], ...]
+    over the distinct values, or 32 equal-width bins [[E_lo, E_hi, count], ...] if there are many."""
+    vals, cnt = np.unique(e, return_counts=True)
+    if vals.size <= 96:
+        return [[int(v), int(c)] for v, c in zip(vals, cnt)]
+    h, edges = np.histogram(e, bins=32)
+    return [[int(edges[i]), int(edges[i + 1]), int(h[i])] for i in range(32)]
+
+
 def cpu_oracle_rate(wl, target_s: float = 20.0):
     """The oracle as it stands, OpenMP over words, on a bounded sample of the workload."""
     from oracle.xs_oracle import NO_HIT, Instance, omp_threads
@@ -326,7 +336,8 @@ def main():
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": int(launches),
             "roofline": roof,
-            "energy": {"mean_per_spin": float(e_np.mean() / N), "min": int(e_np.min()), "max": int(e_np.max())},
+            "energy": {"mean_per_spin": float(e_np.mean() / N), "min": int(e_np.min()), "max": int(e_np.max()),
+                       "histogram": energy_histogram(e_np)},
             "tts": {"solved_instances": int(sum(r.solved for r in recs)), "sweeps_done": int(recs[0].sweeps_done)},
         }
         if not args.no_cpu_baseline:
