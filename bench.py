@@ -302,12 +302,14 @@ def main():
                     "frac": achieved / (alu_peak / 1e3), "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload),
                     "peak_source": "xs_alu_peak LOP3 micro-kernel measured in this run",
                     "peak_nominal_at_sampled_clock": (148 * 64 * clocks["sm_mhz"] / 1e6) if clocks.get("sm_mhz") else None,
-                    "alg_ops_per_update": ALU_OPS_PER_UPDATE, "kernel": "k_sweep_static" if lay.variant == 1 else "k_sweep_tile", "kernel_ms": k_ms}
+                    "alg_ops_per_update": ALU_OPS_PER_UPDATE, "kernel": {1: "k_sweep_static", 2: "k_sweep_clause"}.get(lay.variant, "k_sweep_tile"), "kernel_ms": k_ms}
             # co-limiter: shared-memory pipe, 128 B/clk/SM.  Bytes the kernel's layout
             # moves per update: static kernel 6 loads + NC stores of 16 B per 128 updates (T = 8: two
             # row copies, T = 4: four), generic kernel 11 accesses of 16 B per 128 updates.
             n_copies = 16 // lay.tile_words if lay.tile_words <= 16 else 1            # static kernel: row copies
             sm_bpu = ((6 + n_copies) * 16 / 128.0) if lay.variant == 1 else (11 * 16 / 128.0)
+            if lay.variant == 2:                                                      # clause-word kernel: 3 loads + 3 stores
+                sm_bpu = 6 * 16 / 128.0
             if clocks.get("sm_mhz"):
                 sm_peak = 148 * 128 * clocks["sm_mhz"] / 1e3                          # GB/s
                 roof["shared_memory"] = {"bytes_per_update": sm_bpu,
@@ -329,7 +331,7 @@ def main():
             "data": "synthetic",
             "config": {"workload": wl["desc"], "l2": "flushed between timed iterations (256 MiB write)",
                        "regime": "on-chip" if lay.regime == 0 else "streaming", "tile_words": lay.tile_words,
-                       "threads": lay.threads, "ctas": lay.ctas, "smem_bytes": lay.smem_bytes,
+                       "threads": lay.threads, "ctas": lay.ctas, "smem_bytes": lay.smem_bytes, "kernel_variant": lay.variant,
                        "batch_sweeps": lay.batch_sweeps, "n_sets": lay.n_sets_max, "multi_gpu": "replicas only"},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "clone-spin updates/ns", "h2d_bytes_per_step": h2d,

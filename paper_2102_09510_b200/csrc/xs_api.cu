@@ -51,6 +51,8 @@ DevLayout make_layout(const xs_params& p)
     L.off_seed = o;       o = align_up(o + I * 8, 256);
     L.off_det = o;        o = align_up(o + 2 * I * W * 8, 256);
     L.off_nsets = o;      o = align_up(o + I * 4, 256);
+    L.off_crec = o;       o = align_up(o + I * N * sizeof(CRec), 256);
+    L.off_cplace = o;     o = align_up(o + I * N * 4, 256);
     L.total = o;
     return L;
 }
@@ -88,6 +90,8 @@ static int finish_create(xs_batch* b, void* dev_ws, size_t ws_bytes, void* strea
     b->d.run_seed = reinterpret_cast<uint64_t*>(ws + b->lay.off_seed);
     b->d.det = reinterpret_cast<uint64_t*>(ws + b->lay.off_det);
     b->d.n_sets = reinterpret_cast<uint32_t*>(ws + b->lay.off_nsets);
+    b->d.crec = reinterpret_cast<CRec*>(ws + b->lay.off_crec);
+    b->d.cplace = reinterpret_cast<uint32_t*>(ws + b->lay.off_cplace);
 
     // host staging of the tables (pageable; the copies below are synchronous w.r.t. the host)
     std::vector<AdjRec> adj((size_t)I * N);
@@ -141,6 +145,7 @@ static int finish_create(xs_batch* b, void* dev_ws, size_t ws_bytes, void* strea
     }
     std::string err;
     if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
+    if (int e = clause_prepare(*b, stream)) return cuda_fail(e, "clause tables");
     if (int e = launch_init(*b, stream)) return cuda_fail(e, "init kernel");
     if (int e = launch_mark(*b, true, stream)) return cuda_fail(e, "mark kernel");
     if (int e = launch_finalize(*b, 0, stream)) return cuda_fail(e, "finalize kernel");
@@ -246,6 +251,7 @@ int xs_set_flip_table(xs_batch* b, const uint64_t* thr4)
     if (!ft.general) b->p.w1_threshold = ft.lo[1];
     std::string err;
     if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
+    if (int e = clause_prepare(*b, nullptr)) return cuda_fail(e, "clause tables");
     return XS_OK;
 }
 

@@ -48,10 +48,16 @@ struct alignas(16) ClauseRec {
     uint32_t i, j, k, jbit;
 };
 
+// Task record of the clause-word kernel (xs_sweep_clause.cu): shared-memory row offsets of the
+// three clause rows of the spin at entry set * n_slots + slot, and the spin index (16 bytes).
+struct alignas(16) CRec {
+    uint32_t off0, off1, off2, spin;
+};
+
 // Device workspace carved out of the caller's buffer.
 struct DevLayout {
     size_t off_x = 0, off_first_hit = 0, off_adj = 0, off_clause = 0, off_set_start = 0,
-           off_rec = 0, off_seed = 0, off_det = 0, off_nsets = 0, total = 0;
+           off_rec = 0, off_seed = 0, off_det = 0, off_nsets = 0, off_crec = 0, off_cplace = 0, total = 0;
 };
 DevLayout make_layout(const xs_params& p);
 
@@ -65,6 +71,8 @@ struct DevPtrs {
     uint64_t* run_seed;    // [I]
     uint64_t* det;         // [I][W]   scratch: OR of unsatisfied-clause words
     uint32_t* n_sets;      // [I]
+    CRec* crec;            // [I][N]   clause-word kernel: tasks in slot order
+    uint32_t* cplace;      // [I][N]   clause-word kernel: shared-memory row offset of clause t
 };
 
 // Flip table w_0..w_3 as 32-bit thresholds: a spin with k unsatisfied
@@ -89,7 +97,7 @@ struct TileGeom {
     uint32_t smem = 0;
     uint32_t batch = 0;        // sweeps between in-kernel ground-state checks
     uint32_t rb = 0;           // sweeps of random bytes produced at a time
-    uint32_t variant = 0;      // 0 generic tile kernel, 1 static-task kernel
+    uint32_t variant = 0;      // 0 generic tile kernel, 1 static-task kernel, 2 clause-word kernel
 };
 
 }  // namespace xs
@@ -104,6 +112,8 @@ struct xs_batch {
     xs::FlipTable ft{};
     uint32_t n_sets_max = 0;
     uint32_t max_set_size = 0;
+    uint32_t clause_state = 0;    // clause-word kernel tables: 0 not built, 1 uploaded, 2 not eligible
+    uint32_t clause_slots = 0;    // slots per CTA the uploaded tables were built for
     uint64_t sweeps_issued = 0;   // upper bound on any instance's sweep counter (overflow guard)
     void* ws = nullptr;
 };
@@ -121,4 +131,8 @@ bool static_feasible(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t thread
 uint32_t static_rounds(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t threads);
 uint32_t static_smem_bytes(uint32_t N, uint32_t T);
 int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream);
+// clause-word variant (xs_sweep_clause.cu)
+bool clause_placement(const HostGraph& g, uint32_t n_slots, CRec* crec, uint32_t* cplace);
+int clause_prepare(xs_batch& b, void* stream);
+int launch_sweep_clause(const xs_batch& b, uint32_t n_sweeps, void* stream);
 }  // namespace xs

@@ -1,0 +1,100 @@
+"""GPU-vs-oracle parity of the clause-word kernel (`k_sweep_clause`, layout variant 2): shared
+memory holds c_t = x_i ^ x_j ^ x_k ^ J_t (the number of unsatisfied interactions
+a spin enters is all its update needs), the spin words live in registers.  The kernel serves the
+balanced-set shapes with 4 sets that fill the CTA (bench.py's config 2 / config 3 geometry); results
+must equal the oracle's bit for bit, like every other kernel's."""
+import numpy as np
+import pytest
+import torch
+
+from _harness import OracleRun
+from oracle.xs_oracle import NO_HIT
+from test_gpu_parity import _compare, _xs, env
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(autouse=True)
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
+
+
+@pytest.mark.parametrize("N,W,threads,batch", [
+    (128, 16, 128, 16),     # 4 sets of 32, two tiles
+    (256, 8, 256, 16),      # the config-2 tile
+    (256, 24, 256, 64),     # three tiles, default detection batch
+    (512, 8, 512, 5),       # the config-3 tile, odd batch
+])
+def test_clause_kernel_parity_all_words(N, W, threads, batch):
+    xs = _xs()
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED
+    with env(XS_TILE_WORDS=8, XS_VARIANT=1, XS_BATCH=batch):
+        ref = xs.Batch(N, W, [N + 3], [7 * N], flags=fl)          # spin-word static kernel
+    with env(XS_TILE_WORDS=8, XS_BATCH=batch):    # few tiles: the automatic rule would take T = 4
+        b = xs.Batch(N, W, [N + 3], [7 * N], flags=fl)
+    lay = b.layout()
+    assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == (0, 2, 8, threads)
+    assert ref.layout().variant == 1
+    o = OracleRun(N, W, N + 3, 7 * N, no_skip=True, balanced=True)
+    for n in (1, 2, 40, 23):                 # odd starts of the 2-sweep noise period, resume across calls
+        b.run_sweeps(n)
+        ref.run_sweeps(n)
+        o.run_sweeps(n)
+    _compare(b, [o], f"clause kernel N={N} W={W}")
+    assert np.array_equal(b.spins_numpy(), ref.spins_numpy())
+    b.close()
+    ref.close()
+
+
+@pytest.mark.parametrize("batch", [1, 7, 64])
+def test_clause_kernel_first_hit_many_solved_clones(batch):
+    """Clones started a few spin flips away from the planted state reach E = -N within a few
+    sweeps at different times: detection pass, replay of the batch, exact first-hit sweep (L293)."""
+    xs = _xs()
+    N, W = 128, 8
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED
+    with env(XS_TILE_WORDS=8, XS_BATCH=batch):
+        b = xs.Batch(N, W, [77], [78], flags=fl)
+    assert b.layout().variant == 2
+    o = OracleRun(N, W, 77, 78, no_skip=True, balanced=True)
+    rng = np.random.default_rng(5)
+    taubit = o.inst.taubit.astype(np.uint64)
+    x = np.zeros((1, N, W), np.uint64)
+    x[0] = (taubit * np.uint64(0xFFFFFFFFFFFFFFFF))[:, None]
+    for k in range(64):                       # flip each (spin, clone) bit with probability 0.04
+        x[0] ^= (rng.random((N, W)) < 0.04).astype(np.uint64) << np.uint64(k)
+    b.set_spins(torch.from_numpy(x.view(np.int64)).cuda())
+    o.s = o.inst.unpack(x[0])
+    o.first_hit = o.inst.mark_initial(o.s)
+    for n in (3, 70, 6):
+        b.run_sweeps(n)
+        o.run_sweeps(n)
+    _compare(b, [o], f"clause kernel first hits, batch {batch}")
+    fh = b.first_hit_numpy()[0]
+    hit = fh[fh != NO_HIT]
+    assert hit.size > 50 and np.unique(hit).size > 3      # the case really exercises the replay
+    b.close()
+
+
+def test_clause_kernel_multi_instance_stop_rule_and_flip_table_switch():
+    xs = _xs()
+    N, W, I = 128, 8, 150
+    seeds = [900 + i for i in range(I)]
+    b = xs.Batch(N, W, seeds, seeds, flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_BALANCED)
+    assert b.layout().variant == 2 and b.layout().ctas == I
+    b.set_flip_table([1 << 20, 236223201, 1 << 32, 1 << 32])     # general table: generic kernel
+    assert b.layout().variant == 0
+    b.set_flip_table([0, 236223201, 1 << 32, 1 << 32])           # back to quasi-greedy
+    assert b.layout().variant == 2
+    oracles = {i: OracleRun(N, W, seeds[i], seeds[i], balanced=True) for i in (0, 74, 149)}
+    for n in (33, 64):
+        b.run_sweeps(n)
+    x = b.spins_numpy()
+    fh = b.first_hit_numpy()
+    for i, o in oracles.items():
+        o.run_sweeps(33)
+        o.run_sweeps(64)
+        assert np.array_equal(x[i], o.x()) and np.array_equal(fh[i], o.first_hit)
+    assert all(r.sweeps_done == 97 for r in b.tts())
+    b.close()
