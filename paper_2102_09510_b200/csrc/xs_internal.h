@@ -114,6 +114,7 @@ struct xs_batch {
     uint32_t max_set_size = 0;
     uint32_t clause_state = 0;    // clause-word kernel tables: 0 not built, 1 uploaded, 2 not eligible
     uint32_t clause_slots = 0;    // slots per CTA the uploaded tables were built for
+    uint32_t clause_rounds = 0;   // sets per sweep of those tables (4 or 6)
     uint64_t sweeps_issued = 0;   // upper bound on any instance's sweep counter (overflow guard)
     void* ws = nullptr;
 };

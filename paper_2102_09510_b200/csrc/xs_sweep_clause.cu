@@ -19,7 +19,7 @@
 // touch opposite halves in each of their three accesses (clause_placement below): single copy,
 // conflict free, no second store.
 //
-// Eligibility (clause_prepare): quasi-greedy table, T = 8, 2 words per lane, exactly 4 sets that
+// Eligibility (clause_prepare): quasi-greedy table, T = 8, 2 words per lane, exactly 4 or 6 sets that
 // fill all slots of the CTA (balanced sets, DESIGN.md R-balance).  Everything else runs on
 // k_sweep_static / k_sweep_tile.  The update order inside a set is free (L277), so results are
 // bit-identical to the oracle's.
@@ -38,7 +38,7 @@ void count_launch(uint64_t n);   // xs_diag.cu
 
 namespace {
 
-constexpr int CL_R = 4;        // rounds (= sets) per sweep
+constexpr int CL_RMAX = 6;     // rounds (= sets) per sweep: 4 or 6
 constexpr int CL_H = 4;        // uint32 halves per lane (2 uint64 words)
 constexpr uint32_t CL_T = 8;   // tile width in uint64 columns
 constexpr uint32_t CL_LPS = 4; // lanes per slot
@@ -67,7 +67,7 @@ __device__ __forceinline__ uint32_t prmt_b(uint32_t a, uint32_t b, uint32_t sel)
 }
 constexpr int LUT_OR_AND = 0xF8;   // a | (b & c)
 
-template <int MAXTHREADS, int MINB>
+template <int CL_R, int MAXTHREADS, int MINB>
 __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(ClauseArgs A)
 {
     constexpr uint32_t NL = 2;         // lanes sharing a Philox call = sweeps per noise period
@@ -272,14 +272,23 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(ClauseArgs A)
 inline uint32_t clause_off_misc(uint32_t N) { return N * 128u; }
 inline uint32_t clause_smem(uint32_t N) { return clause_off_misc(N) + (4u * CL_T + 4u) * 4u + 128u; }
 
-template <int MT, int MINB>
+template <int R, int MT, int MINB>
 cudaError_t launch_k(const ClauseArgs& A, uint32_t ctas, uint32_t threads, uint32_t smem, cudaStream_t st)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_clause<MT, MINB>,
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_clause<R, MT, MINB>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_sweep_clause<MT, MINB><<<ctas, threads, smem, st>>>(A);
+    k_sweep_clause<R, MT, MINB><<<ctas, threads, smem, st>>>(A);
     return cudaGetLastError();
+}
+template <int R>
+cudaError_t launch_r(const ClauseArgs& A, const TileGeom& g, cudaStream_t st)
+{
+    const bool dense = g.ctas > 148u;   // more tiles than SMs: cap the registers, 16 warps per SM
+    if (g.threads == 128) return launch_k<R, 128, 4>(A, g.ctas, g.threads, g.smem, st);
+    if (g.threads == 256) return dense ? launch_k<R, 256, 2>(A, g.ctas, g.threads, g.smem, st)
+                                       : launch_k<R, 256, 1>(A, g.ctas, g.threads, g.smem, st);
+    return launch_k<R, 512, 1>(A, g.ctas, g.threads, g.smem, st);
 }
 
 struct Rng {
@@ -294,18 +303,19 @@ struct Rng {
 // accesses.  A spin whose clauses have halves (h1, h2, h3), k ones, pairs with a spin of 3 - k
 // ones: the first lists its clauses by ascending half, the second by descending half.  Needed per
 // set: #(k = 0) = #(k = 3) and #(k = 1) = #(k = 2); found by a randomised local search over
-// half[] (8 constraints for 4 sets, N free bits).  All integer, deterministic.
+// half[] (2 constraints per set, N free bits).  All integer, deterministic.
 // crec[e] = (row offset of clause 1, 2, 3, spin) for entry e = set * n_slots + slot;
 // cplace[t] = row offset of clause t.  Returns false if the instance is not eligible.
 bool clause_placement(const HostGraph& g, uint32_t n_slots, CRec* crec, uint32_t* cplace)
 {
     const uint32_t N = g.n;
-    if (g.set_start.size() != (size_t)CL_R + 1 || (n_slots & 1u) || N != CL_R * n_slots) return false;
+    const int CL_R = (int)g.set_start.size() - 1;
+    if ((CL_R != 4 && CL_R != 6) || (n_slots & 1u) || N != (uint32_t)CL_R * n_slots) return false;
     for (int s = 0; s < CL_R; ++s)
         if (g.set_start[s + 1] - g.set_start[s] != n_slots) return false;
     std::vector<uint8_t> set_of(N), half(N), k(N, 0);
     for (uint32_t pos = 0; pos < N; ++pos) set_of[g.order[pos]] = (uint8_t)(pos / n_slots);
-    int cnt[CL_R][4] = {};
+    int cnt[CL_RMAX][4] = {};
     Rng rng{0x9E3779B97F4A7C15ull ^ ((uint64_t)N << 32) ^ g.tri[0] ^ ((uint64_t)g.tri[1] << 16)};
     for (uint32_t t = 0; t < N; ++t) half[t] = (uint8_t)(rng.next() & 1u);
     for (uint32_t v = 0; v < N; ++v) {
@@ -396,6 +406,7 @@ int clause_prepare(xs_batch& b, void* stream)
         if (e != cudaSuccess) return (int)e;
         b.clause_state = 1;
         b.clause_slots = n_slots;
+        b.clause_rounds = (uint32_t)b.graphs[0].set_start.size() - 1;   // equal for all instances (N = rounds x slots)
     }
     g.variant = 2;
     g.smem = clause_smem(N);
@@ -411,12 +422,7 @@ int launch_sweep_clause(const xs_batch& b, uint32_t n_sweeps, void* stream)
     A.thr = b.p.w1_threshold; A.flags = b.p.flags; A.batch = g.batch;
     A.off_misc = clause_off_misc(b.p.n_spins);
     cudaStream_t st = (cudaStream_t)stream;
-    const bool dense = g.ctas > 148u;   // more tiles than SMs: cap the registers, 16 warps per SM
-    cudaError_t e;
-    if (g.threads == 128) e = launch_k<128, 4>(A, g.ctas, g.threads, g.smem, st);
-    else if (g.threads == 256) e = dense ? launch_k<256, 2>(A, g.ctas, g.threads, g.smem, st)
-                                         : launch_k<256, 1>(A, g.ctas, g.threads, g.smem, st);
-    else e = launch_k<512, 1>(A, g.ctas, g.threads, g.smem, st);
+    const cudaError_t e = b.clause_rounds == 6 ? launch_r<6>(A, g, st) : launch_r<4>(A, g, st);
     if (e != cudaSuccess) return (int)e;
     count_launch(1);
     return 0;

@@ -1,7 +1,7 @@
 """GPU-vs-oracle parity of the clause-word kernel (`k_sweep_clause`, layout variant 2): shared
 memory holds c_t = x_i ^ x_j ^ x_k ^ J_t (the number of unsatisfied interactions
 a spin enters is all its update needs), the spin words live in registers.  The kernel serves the
-balanced-set shapes with 4 sets that fill the CTA (bench.py's config 2 / config 3 geometry); results
+balanced-set shapes with 4 or 6 sets that fill the CTA (bench.py's config 2 / config 3 geometry); results
 must equal the oracle's bit for bit, like every other kernel's."""
 import numpy as np
 import pytest
@@ -25,6 +25,9 @@ def _need_gpu():
     (256, 8, 256, 16),      # the config-2 tile
     (256, 24, 256, 64),     # three tiles, default detection batch
     (512, 8, 512, 5),       # the config-3 tile, odd batch
+    (192, 8, 128, 16),      # 6 sets of 32 (6 rounds per sweep)
+    (384, 16, 256, 64),     # 6 sets of 64
+    (768, 8, 512, 9),       # 6 sets of 128
 ])
 def test_clause_kernel_parity_all_words(N, W, threads, batch):
     xs = _xs()

@@ -90,8 +90,8 @@ def test_config4_shapes_balanced_static_geometry(N, threads, tile):
     seeds = [1000 * N + i for i in range(I)]
     b = xs.Batch(N, W, seeds, seeds, flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED)
     lay = b.layout()
-    # 4 sets that fill the CTA -> clause-word kernel (variant 2), else the spin-word static kernel
-    assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == (0, 2 if N in (128, 256) else 1, tile, threads)
+    # 4 or 6 sets that fill a T = 8 CTA -> clause-word kernel (variant 2); N = 1024 (T = 4): spin-word static kernel
+    assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == (0, 2 if tile == 8 else 1, tile, threads)
     oracles = {i: OracleRun(N, W, seeds[i], seeds[i], no_skip=True, balanced=True) for i in (0, 101, 159)}
     for n in (65, 40):
         b.run_sweeps(n)
