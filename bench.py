@@ -66,7 +66,7 @@ STREAM_BYTES_PER_UPDATE = (8 * 8 * 16 + 28) / 1024.0   # config 5, W=16: 1052 B 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu
 # --set full captures summarised in profiles/r01_ncu_summary.md and r01b_ncu_summary.md (config5: the launch of the
 # largest independent set, 262,053 spin rows = 275.7 MB algorithmic).
-NCU_DRAM_BYTES_PER_LAUNCH = {"config2": 2.42e6, "config2_greedy": 2.43e6, "config3": 93.3e6, "config3_greedy": 91.6e6, "config5": 187.9e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"config2": 2.41e6, "config2_greedy": 2.43e6, "config3": 94.7e6, "config3_greedy": 91.6e6, "config5": 187.9e6}
 
 
 class ClockSampler:
