@@ -9,8 +9,8 @@
 // word's noise mask R, k = 0 never: L65, L101), and flipping the spin toggles its three clauses:
 // c_r ^= flip, x ^= flip.  The spin words themselves live only in the registers of the thread
 // that owns the spin (and in global memory at batch boundaries).  Per task (128 clones of one
-// spin): 3 LDS.128 + 3 STS.128 and 6 logic operations per 32 clones, against 6 + 2 accesses and
-// 7 operations of the spin-word kernel.  Spins of one independent set share no clause (L277),
+// spin): 3 LDS.128 + 3 STS.128 against the 6 + 2 accesses of the spin-word kernel, and the same 7
+// logic operations per 32 clones.  Spins of one independent set share no clause (L277),
 // so the read-modify-write of the clause rows is race free inside a round.
 //
 // Bank conflicts: a T = 8 clause row is 64 B = half of a 128-byte line, and the 8 lanes of one
