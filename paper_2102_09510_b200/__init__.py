@@ -12,7 +12,7 @@ from ._binding import (XS_FLAG_BALANCED, XS_FLAG_CLONE_NOISE, XS_FLAG_GAUGE, XS_
                        XS_W1_THRESHOLD_DEFAULT, XsError, lib, make_params, xs_alu_peak, xs_cavity_barrier,
                        xs_create_instance, xs_kernel_launches,
                        xs_create_instance_from_arrays, xs_destroy, xs_energy, xs_get_first_hit,
-                       xs_generate_graph, xs_get_graph, xs_get_layout, xs_get_spins, xs_params, xs_run_sweeps, xs_set_flip_table,
+                       xs_clause_placement, xs_generate_graph, xs_get_graph, xs_get_layout, xs_get_spins, xs_params, xs_run_sweeps, xs_set_flip_table,
                        xs_set_spins, xs_tts, xs_tts_rec, xs_tts_stats, xs_workspace_bytes)
 
 

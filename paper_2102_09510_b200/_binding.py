@@ -37,7 +37,7 @@ class xs_layout(C.Structure):
 
 EXPORTS = ["xs_workspace_bytes", "xs_create_instance", "xs_create_instance_from_arrays",
            "xs_run_sweeps", "xs_set_flip_table", "xs_energy", "xs_tts", "xs_get_spins", "xs_set_spins",
-           "xs_get_first_hit", "xs_get_graph", "xs_generate_graph", "xs_get_layout", "xs_tts_stats",
+           "xs_get_first_hit", "xs_get_graph", "xs_generate_graph", "xs_clause_placement", "xs_get_layout", "xs_tts_stats",
            "xs_cavity_barrier", "xs_alu_peak", "xs_kernel_launches", "xs_destroy",
            "xs_last_error"]
 
@@ -69,6 +69,7 @@ def lib():
     L.xs_get_graph.argtypes = [vp, C.c_uint32, u32p, u8p, u32p, u32p, u32p]
     L.xs_generate_graph.argtypes = [C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32, u32p, u8p, u32p,
                                     u32p, u32p, C.POINTER(C.c_int32)]
+    L.xs_clause_placement.argtypes = [C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, u32p, u32p]
     L.xs_get_layout.argtypes = [vp, C.POINTER(xs_layout)]
     L.xs_tts_stats.argtypes = [u32p, C.c_uint32, C.c_uint64, C.POINTER(C.c_double)]
     L.xs_cavity_barrier.argtypes = [C.c_uint32, C.c_double, C.POINTER(C.c_double)]
@@ -209,6 +210,16 @@ def xs_generate_graph(n_spins: int, graph_seed: int, flags: int = XS_FLAG_GAUGE,
                                    _ptr(order, C.c_uint32), _ptr(ss, C.c_uint32), C.byref(ns),
                                    C.byref(att)), "xs_generate_graph")
     return tri, jbit, order, ss[: ns.value].copy(), int(att.value)
+
+
+def xs_clause_placement(n_spins: int, graph_seed: int, n_slots: int, flags: int = XS_FLAG_GAUGE | XS_FLAG_BALANCED,
+                        set_cap: int = 0):
+    """Host only.  Returns (task [N][4], place [N]) of the clause-word kernel (include/xs.h)."""
+    task = np.zeros((n_spins, 4), np.uint32)
+    place = np.zeros(n_spins, np.uint32)
+    _check(lib().xs_clause_placement(n_spins, int(graph_seed), int(flags), int(set_cap), int(n_slots),
+                                     _ptr(task, C.c_uint32), _ptr(place, C.c_uint32)), "xs_clause_placement")
+    return task, place
 
 
 def xs_get_layout(h) -> xs_layout:

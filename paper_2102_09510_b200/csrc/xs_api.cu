@@ -319,6 +319,28 @@ int xs_get_graph(const xs_batch* b, uint32_t inst, uint32_t* tri, uint8_t* jbit,
     return XS_OK;
 }
 
+int xs_clause_placement(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uint32_t set_cap,
+                        uint32_t n_slots, uint32_t* task, uint32_t* place)
+{
+    if (n_spins < 3 || n_spins >= (1u << 24)) return fail(XS_EINVAL, "n_spins out of range");
+    try {
+        HostGraph g;
+        std::string err;
+        if (!build_graph_from_seed(n_spins, graph_seed, (flags & XS_FLAG_GAUGE) != 0, set_cap,
+                                   (flags & XS_FLAG_BALANCED) != 0, g, err))
+            return fail(XS_EINVAL, err);
+        std::vector<CRec> crec(n_spins);
+        std::vector<uint32_t> cplace(n_spins);
+        if (!clause_placement(g, n_slots, crec.data(), cplace.data()))
+            return fail(XS_EINVAL, "instance not eligible for the clause-word kernel or no placement found");
+        if (task) std::memcpy(task, crec.data(), (size_t)n_spins * sizeof(CRec));
+        if (place) std::memcpy(place, cplace.data(), (size_t)n_spins * 4);
+    } catch (const std::bad_alloc&) {
+        return fail(XS_ENOMEM, "host allocation failed");
+    }
+    return XS_OK;
+}
+
 int xs_generate_graph(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uint32_t set_cap,
                       uint32_t* tri, uint8_t* jbit, uint32_t* order, uint32_t* set_size,
                       uint32_t* n_sets, int32_t* attempt)

@@ -74,6 +74,44 @@ def test_balanced_sets_match_oracle(N, seed, cap):
         assert np.array_equal(order, g.order)
 
 
+@pytest.mark.parametrize("N,seed,n_slots", [(256, 2, 64), (128, 100, 32), (512, 101, 128), (512, 355, 128),
+                                            (192, 7, 32), (384, 8, 64), (768, 9, 128), (128, 128004, 32),
+                                            (64, 5, 16)])
+def test_clause_placement_is_conflict_free_and_complete(N, seed, n_slots):
+    """Placement tables of the clause-word kernel (include/xs.h), checked straight
+    from the triplets: every set's entries are exactly the set's spins (L277: any order inside a
+    set is valid), an entry's three rows are the three interactions the spin enters (L67), and
+    the two slots of a shared-memory phase touch opposite halves of their 128-byte lines."""
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_BALANCED
+    tri, jbit, order, ss, att = xs.xs_generate_graph(N, seed, fl, 0)
+    assert len(ss) in (4, 6) and (ss == n_slots).all()
+    task, place = xs.xs_clause_placement(N, seed, n_slots, fl, 0)
+    t = np.arange(N, dtype=np.uint32)
+    assert np.array_equal(place & ~np.uint32(64), t << 7)                 # own line, lower or upper half
+    clauses_of = [[] for _ in range(N)]
+    for c, (i, j, k) in enumerate(tri.tolist()):
+        for v in (i, j, k):
+            clauses_of[v].append(c)
+    for s in range(len(ss)):
+        ent = task[s * n_slots:(s + 1) * n_slots]
+        assert sorted(ent[:, 3].tolist()) == sorted(order[s * n_slots:(s + 1) * n_slots].tolist())
+        for e in ent:
+            assert sorted((e[:3] >> 7).tolist()) == sorted(clauses_of[int(e[3])])
+            assert np.array_equal(e[:3], place[e[:3] >> 7])
+        half = (ent[:, :3] >> 6) & 1
+        assert ((half[0::2] ^ half[1::2]) == 1).all()
+    # deterministic
+    task2, place2 = xs.xs_clause_placement(N, seed, n_slots, fl, 0)
+    assert np.array_equal(task, task2) and np.array_equal(place, place2)
+
+
+def test_clause_placement_rejects_ineligible_shapes():
+    with pytest.raises(xs.XsError):                     # greedy sets: ragged
+        xs.xs_clause_placement(256, 2, 64, xs.XS_FLAG_GAUGE, 0)
+    with pytest.raises(xs.XsError):                     # sets of 64 on 32 slots
+        xs.xs_clause_placement(256, 2, 32)
+
+
 def test_workspace_bytes_and_param_errors():
     p = xs.make_params(256, 1024, 1)
     n = xs.xs_workspace_bytes(p)
