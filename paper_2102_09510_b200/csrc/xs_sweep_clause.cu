@@ -288,6 +288,7 @@ cudaError_t launch_r(const ClauseArgs& A, const TileGeom& g, cudaStream_t st)
     if (g.threads == 128) return launch_k<R, 128, 4>(A, g.ctas, g.threads, g.smem, st);
     if (g.threads == 256) return dense ? launch_k<R, 256, 2>(A, g.ctas, g.threads, g.smem, st)
                                        : launch_k<R, 256, 1>(A, g.ctas, g.threads, g.smem, st);
+    if (g.threads == 1024) return launch_k<R, 1024, 1>(A, g.ctas, g.threads, g.smem, st);
     return launch_k<R, 512, 1>(A, g.ctas, g.threads, g.smem, st);
 }
 
@@ -381,12 +382,19 @@ int clause_prepare(xs_batch& b, void* stream)
     TileGeom& g = b.geom;
     const char* env = std::getenv("XS_VARIANT");
     if (env && *env && std::atoi(env) != 2) return 0;        // 0 / 1: experiments with the other kernels
-    if (g.regime != 0 || g.variant != 1 || g.T != CL_T || g.CW != 2 || b.ft.general || b.ft.per_clone)
-        return 0;
+    if (g.regime != 0 || g.variant != 1 || g.CW != 2 || b.ft.general || b.ft.per_clone) return 0;
     if (b.clause_state == 2) return 0;                        // placement failed earlier
     const uint32_t N = b.p.n_spins, I = b.p.n_instances;
-    const uint32_t n_slots = g.threads / CL_LPS;
-    if (g.threads != 128 && g.threads != 256 && g.threads != 512) return 0;
+    uint32_t threads = g.threads;
+    if (g.T == 4 && b.p.n_words % CL_T == 0 && b.max_set_size == 256) {
+        // sets of 256 spins (N = 1024): the static kernel runs them on T = 4 tiles with 512 threads;
+        // here one 1024-thread CTA (32 warps, 64 registers) keeps a T = 8 tile
+        threads = 1024;
+    } else if (g.T != CL_T) {
+        return 0;
+    }
+    const uint32_t n_slots = threads / CL_LPS;
+    if (threads != 128 && threads != 256 && threads != 512 && threads != 1024) return 0;
     if (clause_smem(N) > 227u * 1024u) return 0;
     if (b.clause_state == 0 || b.clause_slots != n_slots) {
         std::vector<CRec> crec((size_t)I * N);
@@ -409,6 +417,9 @@ int clause_prepare(xs_batch& b, void* stream)
         b.clause_rounds = (uint32_t)b.graphs[0].set_start.size() - 1;   // equal for all instances (N = rounds x slots)
     }
     g.variant = 2;
+    g.T = CL_T;
+    g.threads = threads;
+    g.ctas = I * (b.p.n_words / CL_T);
     g.smem = clause_smem(N);
     return 0;
 }

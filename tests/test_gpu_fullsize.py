@@ -81,7 +81,7 @@ def test_config3_shape_sampled_instances_and_words(balanced):
 
 
 @pytest.mark.parametrize("N,threads,tile", [(128, 128, 8), (192, 128, 8), (256, 256, 8), (384, 256, 8),
-                                            (768, 512, 8), (1024, 512, 4)])
+                                            (768, 512, 8), (1024, 1024, 8)])
 def test_config4_shapes_balanced_static_geometry(N, threads, tile):
     """configs[3] shapes that run on the static kernel in bench.py (--workload config4_N): 160
     instances of W = 8 give one tile per SM and more; sampled instances, all words."""
