@@ -417,6 +417,10 @@ int clause_prepare(xs_batch& b, void* stream)
         b.clause_rounds = (uint32_t)b.graphs[0].set_start.size() - 1;   // equal for all instances (N = rounds x slots)
     }
     g.variant = 2;
+    // detection pass + tile store every 256 sweeps (measured +3 % over 64; a replay, which happens
+    // when a clone first reaches E = -N, re-runs at most one batch).  XS_BATCH overrides.
+    const char* eb = std::getenv("XS_BATCH");
+    if (!(eb && *eb)) g.batch = 256;
     g.T = CL_T;
     g.threads = threads;
     g.ctas = I * (b.p.n_words / CL_T);
