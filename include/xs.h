@@ -100,8 +100,24 @@ typedef struct {
     uint32_t smem_bytes;     /* dynamic shared memory per CTA                                    */
     uint32_t batch_sweeps;   /* sweeps between ground-state checks inside the kernel             */
     uint32_t n_sets_max;     /* largest number of independent sets over the instances            */
-    uint32_t variant;        /* on-chip: 0 = generic tile kernel, 1 = static-task kernel         */
+    uint32_t variant;        /* on-chip: 0 = generic tile kernel, 1 = static-task (spin-word)
+                                kernel, 2 = clause-word kernel, 3 = single-warp latency kernel  */
 } xs_layout;
+
+/* Explicit launch geometry (xs_set_geometry).  Every field is a request: 0 (XS_GEOM_AUTO for
+ * `variant`) leaves the choice to the library's rule (DESIGN.md section 7 "Geometry rule"); a
+ * request the shape cannot satisfy (e.g. a tile that does not fit in shared memory, a kernel
+ * that does not take the update order) falls back to the rule for that field, and
+ * xs_get_layout reports what was chosen.  All geometries give bit-identical results. */
+#define XS_GEOM_AUTO 0xFFFFFFFFu
+typedef struct {
+    uint32_t variant;        /* XS_GEOM_AUTO or the on-chip kernel to prefer (xs_layout.variant)  */
+    uint32_t tile_words;     /* T: 1, 2, 4, ... 64 uint64 columns per CTA tile                    */
+    uint32_t threads;        /* threads per CTA, multiple of 32, <= 1024                          */
+    uint32_t words_per_lane; /* static-task kernel: 1 or 2 uint64 words per lane                  */
+    uint32_t batch_sweeps;   /* sweeps between in-kernel ground-state checks (>= 1)               */
+    uint32_t noise_sweeps;   /* generic kernel: sweeps of noise bytes produced at a time (>= 1)   */
+} xs_geometry;
 
 /* Bytes of device workspace a batch with these parameters needs (state, first-hit table,
  * graph tables, per-instance records).  Host call, no CUDA work. */
@@ -143,8 +159,16 @@ int xs_run_sweeps(xs_batch* b, uint64_t n_sweeps, void* cuda_stream);
  * the same u serves every k (L87).  Takes effect from the next xs_run_sweeps; the default after
  * xs_create_instance* is (0, w1_threshold, 2^32, 2^32).  Tables that are not of the quasi-greedy
  * form run on the generic / streaming kernels; with thr4[0] > 0 a ground state can be left
- * again, so first hits are looked for after every sweep.  Host call, no CUDA work. */
-int xs_set_flip_table(xs_batch* b, const uint64_t* thr4);
+ * again, so first hits are looked for after every sweep.  The launch geometry is chosen anew
+ * (a table can move the batch to another kernel); tables a kernel needs are uploaded on
+ * cuda_stream, which is synchronised if an upload happens. */
+int xs_set_flip_table(xs_batch* b, const uint64_t* thr4, void* cuda_stream);
+
+/* Overrides the automatic launch geometry (see xs_geometry); g = NULL restores the rule.
+ * XS_EINVAL for malformed requests (tile_words not a power of two <= 64, threads not a multiple
+ * of 32 or > 1024, words_per_lane > 2).  Takes effect from the next xs_run_sweeps; uploads kernel
+ * tables on cuda_stream like xs_set_flip_table. */
+int xs_set_geometry(xs_batch* b, const xs_geometry* g, void* cuda_stream);
 
 /* a-11.  E_c = -sum_t J_t s_i s_j s_k (L41) for every clone: dev_out [inst][64 W] int32. */
 int xs_energy(xs_batch* b, int32_t* dev_out, void* cuda_stream);
@@ -192,7 +216,9 @@ int xs_clause_placement(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, u
 int xs_get_layout(const xs_batch* b, xs_layout* out);
 
 /* a-12.  TTS statistics "as the paper defines" (L103-L149) over n_runs runs of one instance
- * with sweep cap t_max: tts[r] = TTS in sweeps or XS_NO_HIT (censored).  Host only.
+ * with sweep cap t_max: tts[r] = TTS in sweeps or XS_NO_HIT (censored).  t_max = 0 means the runs
+ * had no cap; XS_EINVAL if an entry is XS_NO_HIT then (a censored run needs its censoring time).
+ * Host only.
  *   out[0] = n (solved runs)                     out[1] = T_tot = sum_solved tts + (n_runs-n) t_max
  *   out[2] = tau_hat = T_tot / n (L139-L147: maximum of the posterior's likelihood; inf if n=0)
  *   out[3..5] = model TTS_50/90/99 = -ln(1-p) tau_hat (L117, L123)

@@ -35,8 +35,15 @@ class xs_layout(C.Structure):
                 ("n_sets_max", C.c_uint32), ("variant", C.c_uint32)]
 
 
+class xs_geometry(C.Structure):
+    _fields_ = [("variant", C.c_uint32), ("tile_words", C.c_uint32), ("threads", C.c_uint32),
+                ("words_per_lane", C.c_uint32), ("batch_sweeps", C.c_uint32), ("noise_sweeps", C.c_uint32)]
+
+
+XS_GEOM_AUTO = 0xFFFFFFFF
+
 EXPORTS = ["xs_workspace_bytes", "xs_create_instance", "xs_create_instance_from_arrays",
-           "xs_run_sweeps", "xs_set_flip_table", "xs_energy", "xs_tts", "xs_get_spins", "xs_set_spins",
+           "xs_run_sweeps", "xs_set_flip_table", "xs_set_geometry", "xs_energy", "xs_tts", "xs_get_spins", "xs_set_spins",
            "xs_get_first_hit", "xs_get_graph", "xs_generate_graph", "xs_clause_placement", "xs_get_layout", "xs_tts_stats",
            "xs_cavity_barrier", "xs_alu_peak", "xs_kernel_launches", "xs_destroy",
            "xs_last_error"]
@@ -60,7 +67,8 @@ def lib():
     L.xs_create_instance_from_arrays.argtypes = [C.POINTER(vp), pp, u32p, u8p, u32p, u32p, u32p,
                                                  C.c_uint32, u64p, vp, C.c_size_t, vp]
     L.xs_run_sweeps.argtypes = [vp, C.c_uint64, vp]
-    L.xs_set_flip_table.argtypes = [vp, u64p]
+    L.xs_set_flip_table.argtypes = [vp, u64p, vp]
+    L.xs_set_geometry.argtypes = [vp, C.POINTER(xs_geometry), vp]
     L.xs_energy.argtypes = [vp, vp, vp]
     L.xs_tts.argtypes = [vp, C.POINTER(xs_tts_rec), vp]
     L.xs_get_spins.argtypes = [vp, vp, vp]
@@ -106,7 +114,7 @@ def _ptr(a, ct):
 
 
 def _stream(stream):
-    """cudaStream_t of a torch stream (None -> torch's current stream)."""
+    """cudaStream_t of a torch stream (None -> torch's current stream on the current device)."""
     import torch
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
@@ -158,10 +166,18 @@ def xs_run_sweeps(h, n_sweeps: int, stream=None):
     _check(lib().xs_run_sweeps(h, int(n_sweeps), _stream(stream)), "xs_run_sweeps")
 
 
-def xs_set_flip_table(h, thr4):
+def xs_set_flip_table(h, thr4, stream=None):
     t = _np(thr4, np.uint64)
     assert t.size == 4
-    _check(lib().xs_set_flip_table(h, _ptr(t, C.c_uint64)), "xs_set_flip_table")
+    _check(lib().xs_set_flip_table(h, _ptr(t, C.c_uint64), _stream(stream)), "xs_set_flip_table")
+
+
+def xs_set_geometry(h, variant=None, tile_words=0, threads=0, words_per_lane=0, batch_sweeps=0,
+                    noise_sweeps=0, stream=None):
+    """Explicit launch geometry (include/xs.h xs_geometry); all defaults = the library's rule."""
+    g = xs_geometry(XS_GEOM_AUTO if variant is None else int(variant), int(tile_words), int(threads),
+                    int(words_per_lane), int(batch_sweeps), int(noise_sweeps))
+    _check(lib().xs_set_geometry(h, C.byref(g), _stream(stream)), "xs_set_geometry")
 
 
 def xs_energy(h, dev_out_ptr: int, stream=None):

@@ -81,6 +81,15 @@ static int finish_create(xs_batch* b, void* dev_ws, size_t ws_bytes, void* strea
     if ((reinterpret_cast<uintptr_t>(dev_ws) & 255u) != 0) return fail(XS_EINVAL, "device workspace must be 256-byte aligned");
     char* ws = static_cast<char*>(dev_ws);
     b->ws = dev_ws;
+    {
+        // the device the workspace lives on (the caller's current device at create time)
+        int dev = 0, sms = 0;
+        if (cudaError_t e = cudaGetDevice(&dev)) return cuda_fail((int)e, "cudaGetDevice");
+        if (cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev))
+            return cuda_fail((int)e, "device attribute");
+        b->device = dev;
+        b->num_sms = sms > 0 ? (uint32_t)sms : 148u;
+    }
     b->d.x = reinterpret_cast<uint64_t*>(ws + b->lay.off_x);
     b->d.first_hit = reinterpret_cast<uint32_t*>(ws + b->lay.off_first_hit);
     b->d.adj = reinterpret_cast<AdjRec*>(ws + b->lay.off_adj);
@@ -229,7 +238,7 @@ int xs_run_sweeps(xs_batch* b, uint64_t n_sweeps, void* cuda_stream)
     return XS_OK;
 }
 
-int xs_set_flip_table(xs_batch* b, const uint64_t* thr4)
+int xs_set_flip_table(xs_batch* b, const uint64_t* thr4, void* cuda_stream)
 {
     if (!b || !thr4) return fail(XS_EINVAL, "null argument");
     FlipTable ft{};
@@ -251,7 +260,31 @@ int xs_set_flip_table(xs_batch* b, const uint64_t* thr4)
     if (!ft.general) b->p.w1_threshold = ft.lo[1];
     std::string err;
     if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
-    if (int e = clause_prepare(*b, nullptr)) return cuda_fail(e, "clause tables");
+    if (int e = clause_prepare(*b, cuda_stream)) return cuda_fail(e, "clause tables");
+    return XS_OK;
+}
+
+int xs_set_geometry(xs_batch* b, const xs_geometry* g, void* cuda_stream)
+{
+    if (!b) return fail(XS_EINVAL, "batch is null");
+    xs_geometry rq{XS_GEOM_AUTO, 0, 0, 0, 0, 0};
+    if (g) {
+        rq = *g;
+        if (rq.variant != XS_GEOM_AUTO && rq.variant > 3u) return fail(XS_EINVAL, "unknown kernel variant");
+        if (rq.tile_words > 64u || (rq.tile_words & (rq.tile_words - 1u)))
+            return fail(XS_EINVAL, "tile_words must be a power of two <= 64");
+        if (rq.threads % 32u || rq.threads > 1024u) return fail(XS_EINVAL, "threads must be a multiple of 32, <= 1024");
+        if (rq.words_per_lane > 2u) return fail(XS_EINVAL, "words_per_lane must be 0, 1 or 2");
+    }
+    const xs_geometry old = b->req;
+    b->req = rq;
+    std::string err;
+    if (!choose_geometry(*b, b->geom, err)) {
+        b->req = old;
+        choose_geometry(*b, b->geom, err);
+        return fail(XS_EINVAL, err);
+    }
+    if (int e = clause_prepare(*b, cuda_stream)) return cuda_fail(e, "clause tables");
     return XS_OK;
 }
 

@@ -116,6 +116,9 @@ struct xs_batch {
     uint32_t clause_slots = 0;    // slots per CTA the uploaded tables were built for
     uint32_t clause_rounds = 0;   // sets per sweep of those tables (4 or 6)
     uint64_t sweeps_issued = 0;   // upper bound on any instance's sweep counter (overflow guard)
+    xs_geometry req{XS_GEOM_AUTO, 0, 0, 0, 0, 0};   // xs_set_geometry requests (0 / AUTO = rule)
+    uint32_t num_sms = 148;       // cudaDevAttrMultiProcessorCount of the device the batch lives on
+    int device = 0;               // CUDA device ordinal the workspace belongs to
     void* ws = nullptr;
 };
 

@@ -99,8 +99,8 @@ __global__ void k_mark(DevPtrs d, uint32_t W, uint32_t I, const uint64_t* det, i
 // Bit-sliced vertical counters per thread (multi-spin coding of the count, L87), then expanded.
 // grid = (W, I, clause chunks)
 // ------------------------------------------------------------------------------------------
-constexpr uint32_t EN_THREADS = 128;
-constexpr uint32_t EN_CHUNK = 8192;
+constexpr uint32_t EN_THREADS = 256;
+constexpr uint32_t EN_MAX_CPT = 252;     // clauses per thread: 8 count planes hold <= 255; multiple of 4
 
 __global__ void k_energy_fill(int32_t* out, uint64_t total, int32_t value)
 {
@@ -109,40 +109,64 @@ __global__ void k_energy_fill(int32_t* out, uint64_t total, int32_t value)
         out[e] = value;
 }
 
+// LANES <-> CONSECUTIVE WORDS of a spin row (LW = 2^lw_shift <= 32 of them), so that every gather
+// x[i][w0 .. w0+LW) is one contiguous, fully used 8 LW-byte segment; the 256 / LW lane groups of a
+// CTA take different clauses of the CTA's chunk.  Per thread the unsatisfied-clause count of its
+// word's 64 clones is kept bit-sliced in 8 planes; four clause words enter per step through a
+// carry-save adder tree (full adder = one XOR3 + one MAJ per 32 clones).
+// grid = (word blocks x clause chunks, I)
 __global__ void __launch_bounds__(EN_THREADS) k_energy_acc(DevPtrs d, uint32_t N, uint32_t W,
-                                                          int32_t* out)
+                                                          uint32_t lw_shift, uint32_t wblocks,
+                                                          uint32_t cpt, int32_t* out)
 {
-    __shared__ int cnt[64];
-    const uint32_t w = blockIdx.x, inst = blockIdx.y;
-    const uint32_t c0 = blockIdx.z * EN_CHUNK;
-    const uint32_t c1 = min(c0 + EN_CHUNK, N);
-    if (threadIdx.x < 64) cnt[threadIdx.x] = 0;
+    __shared__ int cnt[32 * 64];
+    const uint32_t inst = blockIdx.y;
+    const uint32_t wblock = blockIdx.x % wblocks, chunk = blockIdx.x / wblocks;
+    const uint32_t LW = 1u << lw_shift, groups = EN_THREADS >> lw_shift;
+    const uint32_t wl = threadIdx.x & (LW - 1u), cg = threadIdx.x >> lw_shift;
+    const uint32_t w = wblock * LW + wl;
+    const bool valid = w < W;
+    for (uint32_t e = threadIdx.x; e < LW * 64u; e += EN_THREADS) cnt[e] = 0;
     __syncthreads();
     const ClauseRec* cl = d.clause + (size_t)inst * N;
-    const uint64_t* x = d.x + (size_t)inst * N * W;
-    // planes[p] holds bit p of the per-clone count; EN_CHUNK / EN_THREADS = 64 clauses per
-    // thread at most -> 7 planes.
-    uint64_t planes[7] = {0, 0, 0, 0, 0, 0, 0};
-    for (uint32_t c = c0 + threadIdx.x; c < c1; c += EN_THREADS) {
+    const uint64_t* x = d.x + (size_t)inst * N * W + (valid ? w : 0u);
+    const uint32_t c_first = chunk * groups * cpt + cg;      // this thread: c_first, + groups, ...
+    auto unsat = [&](uint32_t c) -> uint64_t {
+        if (c >= N || !valid) return 0ull;
         const ClauseRec r = cl[c];
-        uint64_t carry = x[(size_t)r.i * W + w] ^ x[(size_t)r.j * W + w] ^ x[(size_t)r.k * W + w] ^
-                         (r.jbit ? ~0ull : 0ull);
+        return x[(size_t)r.i * W] ^ x[(size_t)r.j * W] ^ x[(size_t)r.k * W] ^ (r.jbit ? ~0ull : 0ull);
+    };
+    uint64_t pl[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (uint32_t q = 0; q < cpt; q += 4) {
+        const uint32_t c = c_first + q * groups;
+        const uint64_t u0 = unsat(c), u1 = unsat(c + groups), u2 = unsat(c + 2 * groups),
+                       u3 = unsat(c + 3 * groups);
+        const uint64_t s1 = u0 ^ u1 ^ u2, c1 = (u0 & u1) | (u2 & (u0 ^ u1));          // weight 1, 2
+        const uint64_t s2 = s1 ^ u3 ^ pl[0], c2 = (s1 & u3) | (pl[0] & (s1 ^ u3));    // weight 1, 2
+        pl[0] = s2;
+        const uint64_t s3 = c1 ^ c2 ^ pl[1];
+        uint64_t carry = (c1 & c2) | (pl[1] & (c1 ^ c2));                             // weight 4
+        pl[1] = s3;
 #pragma unroll
-        for (int p = 0; p < 7; ++p) {
-            const uint64_t s = planes[p] ^ carry;
-            carry &= planes[p];
-            planes[p] = s;
+        for (int p = 2; p < 8; ++p) {
+            const uint64_t t = pl[p] ^ carry;
+            carry &= pl[p];
+            pl[p] = t;
         }
     }
-    for (int b = 0; b < 64; ++b) {
-        int v = 0;
+    if (valid) {
+        for (int b = 0; b < 64; ++b) {
+            int v = 0;
 #pragma unroll
-        for (int p = 0; p < 7; ++p) v |= (int)((planes[p] >> b) & 1ull) << p;
-        if (v) atomicAdd(&cnt[b], v);
+            for (int p = 0; p < 8; ++p) v |= (int)((pl[p] >> b) & 1ull) << p;
+            if (v) atomicAdd(&cnt[wl * 64u + b], v);
+        }
     }
     __syncthreads();
-    if (threadIdx.x < 64 && cnt[threadIdx.x])
-        atomicAdd(out + ((size_t)inst * W + w) * 64 + threadIdx.x, 2 * cnt[threadIdx.x]);
+    int32_t* o = out + ((size_t)inst * W + (size_t)wblock * LW) * 64;
+    const uint32_t n_valid = min(LW, W - wblock * LW) * 64u;
+    for (uint32_t e = threadIdx.x; e < n_valid; e += EN_THREADS)
+        if (cnt[e]) atomicAdd(o + e, 2 * cnt[e]);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -648,14 +672,8 @@ __global__ void k_mark_swept(DevPtrs d, uint32_t W, uint32_t I, const uint64_t* 
 // ------------------------------------------------------------------------------------------
 namespace {
 constexpr uint32_t SMEM_MAX = 227u * 1024u;   // per-CTA opt-in limit on sm_100a
-constexpr uint32_t NUM_SMS = 148;
 
 inline uint32_t round_up(uint32_t v, uint32_t m) { return (v + m - 1) / m * m; }
-inline uint32_t env_u32(const char* name, uint32_t dflt)
-{
-    const char* s = std::getenv(name);
-    return (s && *s) ? (uint32_t)std::strtoul(s, nullptr, 10) : dflt;
-}
 
 struct TileSmem { uint32_t off_rec, off_rbuf, off_sets, off_misc, total; };
 TileSmem tile_smem(uint32_t N, uint32_t T, uint32_t rb, uint32_t n_sets_max)
@@ -675,15 +693,17 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
 {
     const xs_params& p = b.p;
     g = TileGeom{};
-    g.batch = std::max(1u, env_u32("XS_BATCH", 64));
-    const uint32_t force_T = env_u32("XS_TILE_WORDS", 0);
+    const xs_geometry& rq = b.req;                  // explicit requests (xs_set_geometry), 0 = rule
+    const uint32_t NUM_SMS = std::max(1u, b.num_sms);
+    g.batch = rq.batch_sweeps ? rq.batch_sweeps : 64u;
+    const uint32_t force_T = rq.tile_words;
     uint32_t bestT = 0;
     // Measured on B200: with at least one 16-column tile per SM
     // the generic kernel with T = 16 (128-byte rows: conflict-free, several CTAs per SM overlap
     // their load / compute / barrier phases) is the fastest choice; with fewer tiles than SMs
     // (config 2) the static-task kernel with T = 8 wins because one CTA per SM must hide its
-    // own latencies.  XS_VARIANT: unset = this rule, 0 = generic only, 1 = static if feasible.
-    const uint32_t want_variant = env_u32("XS_VARIANT", 2);
+    // own latencies.  xs_geometry.variant: AUTO / 2 = this rule, 0 = generic only, 1 = static if feasible.
+    const uint32_t want_variant = (rq.variant == XS_GEOM_AUTO || rq.variant > 1u) ? 2u : rq.variant;
     const bool many_tiles = (p.n_words % 16 == 0) &&
                             (uint64_t)p.n_instances * (p.n_words / 16) >= NUM_SMS &&
                             tile_smem(p.n_spins, 16, 1, b.n_sets_max).total <= SMEM_MAX;
@@ -720,8 +740,8 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     const bool few_tiles = (uint64_t)p.n_instances * ((p.n_words + 7) / 8) < 2ull * NUM_SMS;
     if (!(p.flags & XS_FLAG_STREAMING) && !b.ft.general &&     // static kernel: quasi-greedy table only
         (want_variant == 1 || (want_variant == 2 && !auto_T && few_tiles))) {
-        const uint32_t force_thr = env_u32("XS_THREADS", 0);
-        const uint32_t force_cw = env_u32("XS_CW", 0);
+        const uint32_t force_thr = rq.threads;
+        const uint32_t force_cw = rq.words_per_lane;
         uint32_t sT = 0, sThr = 0, sCW = 0;
         uint64_t s_cost = ~0ull;
         for (uint32_t T = 64; T >= 4; T >>= 1) {
@@ -795,20 +815,20 @@ bool choose_geometry(const xs_batch& b, TileGeom& g, std::string& err)
     const uint32_t LPS = g.T / g.CW;
     const uint32_t want = round_up(std::max(b.max_set_size, 1u) * LPS, 32);
     g.threads = std::min(1024u, std::max(128u, want));
-    g.threads = std::min(1024u, std::max(32u, env_u32("XS_THREADS", g.threads) / 32 * 32));
+    if (rq.threads) g.threads = std::min(1024u, std::max(32u, rq.threads / 32 * 32));
     g.ctas = p.n_instances * (p.n_words / g.T);
-    uint32_t rb = std::min(g.batch, env_u32("XS_RB", 8));
+    uint32_t rb = std::max(1u, std::min(g.batch, rq.noise_sweeps ? rq.noise_sweeps : 8u));
     while (rb > 1 && tile_smem(p.n_spins, g.T, rb, b.n_sets_max).total > SMEM_MAX) --rb;
     // Two CTAs per SM overlap each other's load / compute / barrier phases (measured +19 % on
     // config 3, profiles/r01_ncu_summary.md): shrink the noise ring and the CTA until two fit
     // (228 KB shared memory and 64 K registers per SM; this kernel uses 56 registers).
-    if (!env_u32("XS_RB", 0) && g.ctas >= 2 * NUM_SMS) {
+    if (!rq.noise_sweeps && g.ctas >= 2 * NUM_SMS) {
         const uint32_t sm_smem = 228u * 1024u, reserved = 1024u;
         uint32_t r2 = rb;
         while (r2 > 1 && 2 * (tile_smem(p.n_spins, g.T, r2, b.n_sets_max).total + reserved) > sm_smem) r2 /= 2;
         if (2 * (tile_smem(p.n_spins, g.T, r2, b.n_sets_max).total + reserved) <= sm_smem) {
             rb = r2;
-            if (!env_u32("XS_THREADS", 0)) g.threads = std::min(g.threads, 512u);
+            if (!rq.threads) g.threads = std::min(g.threads, 512u);
         }
     }
     g.rb = rb;
@@ -826,7 +846,7 @@ void count_launch(uint64_t n);   // xs_diag.cu
 
 static inline uint32_t grid_for(uint64_t total, uint32_t threads)
 {
-    return (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>((total + threads - 1) / threads, NUM_SMS * 16));
+    return (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>((total + threads - 1) / threads, 148u * 16u));
 }
 
 int launch_init(const xs_batch& b, void* stream)
@@ -877,8 +897,18 @@ int launch_energy(const xs_batch& b, int32_t* dev_out, void* stream)
     const uint64_t total = (uint64_t)p.n_instances * p.n_words * 64;
     k_energy_fill<<<grid_for(total, 256), 256, 0, st>>>(dev_out, total, -(int32_t)p.n_spins);
     count_launch(1);
-    dim3 grid(p.n_words, p.n_instances, (p.n_spins + EN_CHUNK - 1) / EN_CHUNK);
-    k_energy_acc<<<grid, EN_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, dev_out);
+    // lanes <-> words: LW = smallest power of two >= W, at most 32
+    uint32_t lw_shift = 0;
+    while (lw_shift < 5 && (1u << lw_shift) < p.n_words) ++lw_shift;
+    const uint32_t LW = 1u << lw_shift, groups = EN_THREADS >> lw_shift;
+    const uint32_t wblocks = (p.n_words + LW - 1) / LW;
+    // clauses per thread: as many as the count planes hold, fewer when that leaves SMs without a CTA
+    const uint64_t want_chunks = std::max<uint64_t>(1, (4ull * b.num_sms) / ((uint64_t)wblocks * p.n_instances));
+    uint64_t cpt = ((uint64_t)p.n_spins + groups * want_chunks - 1) / (groups * want_chunks);
+    cpt = std::min<uint64_t>(EN_MAX_CPT, std::max<uint64_t>(4, (cpt + 3) / 4 * 4));
+    const uint32_t chunks = (uint32_t)(((uint64_t)p.n_spins + groups * cpt - 1) / (groups * cpt));
+    dim3 grid(wblocks * chunks, p.n_instances);
+    k_energy_acc<<<grid, EN_THREADS, 0, st>>>(b.d, p.n_spins, p.n_words, lw_shift, wblocks, (uint32_t)cpt, dev_out);
     count_launch(1);
     return (int)cudaGetLastError();
 }

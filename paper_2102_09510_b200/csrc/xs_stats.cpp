@@ -46,6 +46,11 @@ extern "C" int xs_tts_stats(const uint32_t* tts, uint32_t n_runs, uint64_t t_max
     uint32_t n = 0;
     double t_tot = 0.0;
     std::vector<double> v(n_runs);
+    // t_max = 0 means "no cap": an unsolved run then has no censoring time to contribute and
+    // would silently count as zero cost (tau biased low) -> refuse
+    if (t_max == 0)
+        for (uint32_t r = 0; r < n_runs; ++r)
+            if (tts[r] == XS_NO_HIT) return XS_EINVAL;
     for (uint32_t r = 0; r < n_runs; ++r) {
         const bool solved = tts[r] != XS_NO_HIT && (t_max == 0 || tts[r] <= t_max);
         if (solved) { ++n; t_tot += (double)tts[r]; v[r] = (double)tts[r]; }

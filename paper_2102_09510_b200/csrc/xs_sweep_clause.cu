@@ -282,9 +282,9 @@ cudaError_t launch_k(const ClauseArgs& A, uint32_t ctas, uint32_t threads, uint3
     return cudaGetLastError();
 }
 template <int R>
-cudaError_t launch_r(const ClauseArgs& A, const TileGeom& g, cudaStream_t st)
+cudaError_t launch_r(const ClauseArgs& A, const TileGeom& g, uint32_t num_sms, cudaStream_t st)
 {
-    const bool dense = g.ctas > 148u;   // more tiles than SMs: cap the registers, 16 warps per SM
+    const bool dense = g.ctas > num_sms;   // more tiles than SMs: cap the registers, 16 warps per SM
     if (g.threads == 128) return launch_k<R, 128, 4>(A, g.ctas, g.threads, g.smem, st);
     if (g.threads == 256) return dense ? launch_k<R, 256, 2>(A, g.ctas, g.threads, g.smem, st)
                                        : launch_k<R, 256, 1>(A, g.ctas, g.threads, g.smem, st);
@@ -380,8 +380,7 @@ bool clause_placement(const HostGraph& g, uint32_t n_slots, CRec* crec, uint32_t
 int clause_prepare(xs_batch& b, void* stream)
 {
     TileGeom& g = b.geom;
-    const char* env = std::getenv("XS_VARIANT");
-    if (env && *env && std::atoi(env) != 2) return 0;        // 0 / 1: experiments with the other kernels
+    if (b.req.variant != XS_GEOM_AUTO && b.req.variant != 2u) return 0;   // another kernel was asked for
     if (g.regime != 0 || g.variant != 1 || g.CW != 2 || b.ft.general || b.ft.per_clone) return 0;
     if (b.clause_state == 2) return 0;                        // placement failed earlier
     const uint32_t N = b.p.n_spins, I = b.p.n_instances;
@@ -418,9 +417,8 @@ int clause_prepare(xs_batch& b, void* stream)
     }
     g.variant = 2;
     // detection pass + tile store every 256 sweeps (measured +3 % over 64; a replay, which happens
-    // when a clone first reaches E = -N, re-runs at most one batch).  XS_BATCH overrides.
-    const char* eb = std::getenv("XS_BATCH");
-    if (!(eb && *eb)) g.batch = 256;
+    // when a clone first reaches E = -N, re-runs at most one batch).  xs_geometry.batch_sweeps overrides.
+    if (!b.req.batch_sweeps) g.batch = 256;
     g.T = CL_T;
     g.threads = threads;
     g.ctas = I * (b.p.n_words / CL_T);
@@ -437,7 +435,7 @@ int launch_sweep_clause(const xs_batch& b, uint32_t n_sweeps, void* stream)
     A.thr = b.p.w1_threshold; A.flags = b.p.flags; A.batch = g.batch;
     A.off_misc = clause_off_misc(b.p.n_spins);
     cudaStream_t st = (cudaStream_t)stream;
-    const cudaError_t e = b.clause_rounds == 6 ? launch_r<6>(A, g, st) : launch_r<4>(A, g, st);
+    const cudaError_t e = b.clause_rounds == 6 ? launch_r<6>(A, g, b.num_sms, st) : launch_r<4>(A, g, b.num_sms, st);
     if (e != cudaSuccess) return (int)e;
     count_launch(1);
     return 0;

@@ -74,7 +74,7 @@ int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream)
     StaticLaunch L;
     L.rounds = static_rounds(b, g.T, g.CW, g.threads);
     L.threads = g.threads; L.ctas = g.ctas; L.smem = g.smem;
-    L.dense = g.ctas > 148u;
+    L.dense = g.ctas > b.num_sms;
     // FULL: exactly `rounds` sets, one round each, and the last warp of the CTA has a task in each
     {
         const uint32_t n_slots = g.threads / (g.T / g.CW), slots_per_warp = 32u / (g.T / g.CW);

@@ -158,6 +158,10 @@ def test_tts_stats_closed_forms():
     assert z["n_solved"] == 0 and math.isinf(z["tau_hat"])
     assert z["tau_q16"] == pytest.approx(10 * 1000 / math.log(20.0))
     # n = 1: inverse-gamma(1, T): median = T / ln 2
+    # no cap given (t_max = 0) but a run is censored: no censoring time -> refused, not biased low
+    with pytest.raises(xs.XsError) as ei:
+        xs.xs_tts_stats(np.array([10, xs.XS_NO_HIT, 30], np.uint32), 0)
+    assert ei.value.code == -1
     one = xs.xs_tts_stats(np.array([700], np.uint32), 0)
     assert one["tau_q50"] == pytest.approx(700 / math.log(2.0), rel=1e-9)
 

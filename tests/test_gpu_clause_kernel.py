@@ -9,7 +9,7 @@ import torch
 
 from _harness import OracleRun
 from oracle.xs_oracle import NO_HIT
-from test_gpu_parity import _compare, _xs, env
+from test_gpu_parity import _compare, _xs
 
 pytestmark = pytest.mark.gpu
 
@@ -32,10 +32,10 @@ def _need_gpu():
 def test_clause_kernel_parity_all_words(N, W, threads, batch):
     xs = _xs()
     fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED
-    with env(XS_TILE_WORDS=8, XS_VARIANT=1, XS_BATCH=batch):
-        ref = xs.Batch(N, W, [N + 3], [7 * N], flags=fl)          # spin-word static kernel
-    with env(XS_TILE_WORDS=8, XS_BATCH=batch):    # few tiles: the automatic rule would take T = 4
-        b = xs.Batch(N, W, [N + 3], [7 * N], flags=fl)
+    ref = xs.Batch(N, W, [N + 3], [7 * N], flags=fl,
+                 geometry=dict(tile_words=8, variant=1, batch_sweeps=batch))          # spin-word static kernel
+    b = xs.Batch(N, W, [N + 3], [7 * N], flags=fl,
+                 geometry=dict(tile_words=8, batch_sweeps=batch))    # few tiles: the automatic rule would take T = 4
     lay = b.layout()
     assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == (0, 2, 8, threads)
     assert ref.layout().variant == 1
@@ -57,8 +57,8 @@ def test_clause_kernel_first_hit_many_solved_clones(batch):
     xs = _xs()
     N, W = 128, 8
     fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED
-    with env(XS_TILE_WORDS=8, XS_BATCH=batch):
-        b = xs.Batch(N, W, [77], [78], flags=fl)
+    b = xs.Batch(N, W, [77], [78], flags=fl,
+                 geometry=dict(tile_words=8, batch_sweeps=batch))
     assert b.layout().variant == 2
     o = OracleRun(N, W, 77, 78, no_skip=True, balanced=True)
     rng = np.random.default_rng(5)

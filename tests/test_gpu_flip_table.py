@@ -5,7 +5,6 @@ looked for after every sweep)."""
 from __future__ import annotations
 
 import math
-import os
 
 import numpy as np
 import pytest
@@ -70,11 +69,7 @@ def test_first_hits_with_w0_positive_small_system(streaming):
     import paper_2102_09510_b200 as xs
     N, W, t4 = 14, 4, metropolis(1.5)
     flags = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_STREAMING if streaming else 0)
-    os.environ["XS_BATCH"] = "7"
-    try:
-        b = xs.Batch(N, W, [3], [4], flags=flags)
-    finally:
-        os.environ.pop("XS_BATCH", None)
+    b = xs.Batch(N, W, [3], [4], flags=flags, geometry=dict(batch_sweeps=7))
     b.set_flip_table(t4)
     o = OracleRun(N, W, 3, 4, no_skip=True, thr4=t4)
     for n in (5, 20, 11):

@@ -46,7 +46,7 @@ def test_config2_full_size_sampled_words(balanced):
     words = [0, 7, 8, 517, 1023]          # first/last lane of a tile, tile boundaries, last tile
     o = OracleRun(N, W, 2, 2, set_cap=64 if balanced else 0, no_skip=True, words=words,
                   balanced=balanced)
-    for n in (130, 171):                  # crosses batch boundaries (64) at odd offsets
+    for n in (130, 171):                  # 301 sweeps: crosses one 256-sweep detection batch at odd offsets
         b.run_sweeps(n)
         o.run_sweeps(n)
     _check_words(b, o)
@@ -71,12 +71,13 @@ def test_config3_shape_sampled_instances_and_words(balanced):
     assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == ((0, 2, 8, 512) if balanced else (0, 0, 16, 512))
     checks = {0: [0, 15, 16], 77: [33, 63], 159: [48]}
     oracles = {i: OracleRun(N, W, seeds[i], seeds[i], words=ws, balanced=balanced) for i, ws in checks.items()}
-    b.run_sweeps(70)
+    for n in (70, 563):                   # 633 sweeps: two full 256-sweep detection batches + a remainder
+        b.run_sweeps(n)
     for i, o in oracles.items():
-        o.run_sweeps(70)
+        o.run_sweeps(633)
         _check_words(b, o, inst=i)
     recs = b.tts()
-    assert all(r.sweeps_done == 70 for r in recs)
+    assert all(r.sweeps_done == 633 for r in recs)
     b.close()
 
 
@@ -93,11 +94,61 @@ def test_config4_shapes_balanced_static_geometry(N, threads, tile):
     # 4 or 6 sets that fill a T = 8 CTA -> clause-word kernel (variant 2); N = 1024 (T = 4): spin-word static kernel
     assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == (0, 2 if tile == 8 else 1, tile, threads)
     oracles = {i: OracleRun(N, W, seeds[i], seeds[i], no_skip=True, balanced=True) for i in (0, 101, 159)}
-    for n in (65, 40):
+    for n in (65, 40, 530):               # 635 sweeps: two full 256-sweep detection batches + a remainder
         b.run_sweeps(n)
     for i, o in oracles.items():
-        o.run_sweeps(105)
+        o.run_sweeps(635)
         _check_words(b, o, inst=i)
+    b.close()
+
+
+def test_config2_full_sweep_count_sampled_words():
+    """configs[1] exactly as bench.py runs it: ONE xs_run_sweeps call of 10^4 sweeps (39 detection
+    batches of 256 + 16) on 2^16 clones; sampled words followed by the oracle for all 10^4 sweeps
+    (SURVEY.md 8(c) protocol (ii))."""
+    import paper_2102_09510_b200 as xs
+    N, W = 256, 1024
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED
+    b = xs.Batch(N, W, [2], [2], set_cap=64, flags=fl)
+    lay = b.layout()
+    assert (lay.regime, lay.variant, lay.tile_words, lay.ctas, lay.batch_sweeps) == (0, 2, 8, 128, 256)
+    words = [0, 7, 517, 1023]
+    o = OracleRun(N, W, 2, 2, set_cap=64, no_skip=True, words=words, balanced=True)
+    b.run_sweeps(10_000)
+    o.run_sweeps(10_000)
+    _check_words(b, o)
+    assert b.tts()[0].sweeps_done == 10_000
+    b.close()
+
+
+@pytest.mark.parametrize("clone_noise", [False, True])
+def test_config5_full_size_grid_stride_path(clone_noise):
+    """configs[4] at its real size, N = 2^20, W = 16: the largest independent set has ~262 000 spins
+    x 8 lane tasks, more than the 8 CTAs per SM x 256 threads the launch has, so every thread of
+    k_stream_set loops over several tasks (the path N = 2^16 never reaches).  One sampled word is
+    followed by the oracle (1 GiB of one-byte spins on the host); with XS_FLAG_CLONE_NOISE the
+    per-clone noise variant runs on the same path."""
+    import paper_2102_09510_b200 as xs
+    N, W = 1 << 20, 16
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_CLONE_NOISE if clone_noise else 0)
+    b = xs.Batch(N, W, [5], [5], flags=fl)
+    lay = b.layout()
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    assert lay.regime == 1 and lay.ctas == 8 * sms
+    _, _, _, ss = b.get_graph(0)
+    assert int(ss.max()) * (W // 2) > lay.ctas * lay.threads     # more than one task per thread
+    o = OracleRun(N, W, 5, 5, no_skip=True, words=[9], clone_m=7 if clone_noise else None)
+    b.run_sweeps(2)
+    o.run_sweeps(2)
+    x = b.spins_numpy()[0]
+    assert np.array_equal(x[:, 9], o.x()[:, 9]), "spin words differ"
+    fh = b.first_hit_numpy()[0]
+    assert np.array_equal(fh[576:640], o.first_hit[576:640])
+    e = b.energy().cpu().numpy()[0]
+    s9 = o.s[576:640]
+    assert np.array_equal(e[576:640], o.inst.energy(s9))
+    assert e.min() >= -N and (e % 2 == 0).all()
+    assert b.tts()[0].sweeps_done == 2
     b.close()
 
 

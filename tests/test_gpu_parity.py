@@ -6,8 +6,6 @@ Protocol: SURVEY.md 8(c) "GPU-vs-oracle parity protocol" -- words evolve indepen
 """
 from __future__ import annotations
 
-import os
-
 import numpy as np
 import pytest
 
@@ -28,24 +26,6 @@ def _xs():
 def _need_gpu():
     if not torch.cuda.is_available():
         pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
-
-
-class env:
-    """Temporarily set geometry knobs the library reads at xs_create_instance time."""
-
-    def __init__(self, **kw):
-        self.kw = {k: str(v) for k, v in kw.items()}
-
-    def __enter__(self):
-        self.old = {k: os.environ.get(k) for k in self.kw}
-        os.environ.update(self.kw)
-
-    def __exit__(self, *a):
-        for k, v in self.old.items():
-            if v is None:
-                os.environ.pop(k, None)
-            else:
-                os.environ[k] = v
 
 
 def _compare(b, oracles, what=""):
@@ -92,8 +72,8 @@ def test_init_state_and_energy():
 def test_sweep_parity_all_words(N, W, sweeps, tile, variant):
     """variant 0 = generic tile kernel, 1 = static-task kernel (falls back to 0 when T < 8)."""
     xs = _xs()
-    with env(XS_TILE_WORDS=tile, XS_BATCH=16, XS_VARIANT=variant):
-        b = xs.Batch(N, W, [N + 7], [3 * N + 1], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
+    b = xs.Batch(N, W, [N + 7], [3 * N + 1], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP,
+                 geometry=dict(tile_words=tile, batch_sweeps=16, variant=variant))
     if tile:
         assert b.layout().tile_words == tile and b.layout().regime == 0
         if variant == 0:
@@ -123,8 +103,8 @@ def test_balanced_sets_parity(N, W, cap, tile, variant, streaming):
     fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED
     if streaming:
         fl |= xs.XS_FLAG_STREAMING
-    with env(XS_TILE_WORDS=tile, XS_BATCH=16, XS_VARIANT=variant):
-        b = xs.Batch(N, W, [N + 11], [5 * N + 1], set_cap=cap, flags=fl)
+    b = xs.Batch(N, W, [N + 11], [5 * N + 1], set_cap=cap, flags=fl,
+                 geometry=dict(tile_words=tile, batch_sweeps=16, variant=variant))
     o = OracleRun(N, W, N + 11, 5 * N + 1, set_cap=cap, no_skip=True, balanced=True)
     assert o.inst.balanced
     tri, jbit, order, ss = b.get_graph(0)
@@ -148,8 +128,8 @@ def test_balanced_sets_parity(N, W, cap, tile, variant, streaming):
 def test_static_kernel_one_word_per_lane(N, W, tile, threads, sweeps):
     """Static-task kernel with CW = 1: four lanes share a Philox call over a 4-sweep period."""
     xs = _xs()
-    with env(XS_TILE_WORDS=tile, XS_BATCH=10, XS_VARIANT=1, XS_CW=1, XS_THREADS=threads):
-        b = xs.Batch(N, W, [N + 3], [N + 4], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
+    b = xs.Batch(N, W, [N + 3], [N + 4], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP,
+                 geometry=dict(tile_words=tile, batch_sweeps=10, variant=1, words_per_lane=1, threads=threads))
     lay = b.layout()
     assert (lay.variant, lay.tile_words, lay.threads) == (1, tile, threads)
     o = OracleRun(N, W, N + 3, N + 4, no_skip=True)
@@ -194,8 +174,8 @@ def test_first_hit_exact_many_solved_clones(batch, streaming, W):
     xs = _xs()
     N = 18
     flags = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_STREAMING if streaming else 0)
-    with env(XS_BATCH=batch, XS_VARIANT=(1 if W == 8 else 0)):
-        b = xs.Batch(N, W, [5], [9], flags=flags)
+    b = xs.Batch(N, W, [5], [9], flags=flags,
+                 geometry=dict(batch_sweeps=batch, variant=(1 if W == 8 else 0)))
     assert b.layout().regime == (1 if streaming else 0)
     if not streaming:
         assert b.layout().variant == (1 if W == 8 else 0)
