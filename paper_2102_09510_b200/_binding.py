@@ -77,7 +77,7 @@ def lib():
     L.xs_get_graph.argtypes = [vp, C.c_uint32, u32p, u8p, u32p, u32p, u32p]
     L.xs_generate_graph.argtypes = [C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32, u32p, u8p, u32p,
                                     u32p, u32p, C.POINTER(C.c_int32)]
-    L.xs_clause_placement.argtypes = [C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, u32p, u32p]
+    L.xs_clause_placement.argtypes = [C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, u32p, u32p, u32p, u32p]
     L.xs_get_layout.argtypes = [vp, C.POINTER(xs_layout)]
     L.xs_tts_stats.argtypes = [u32p, C.c_uint32, C.c_uint64, C.POINTER(C.c_double)]
     L.xs_cavity_barrier.argtypes = [C.c_uint32, C.c_double, C.POINTER(C.c_double)]
@@ -230,12 +230,15 @@ def xs_generate_graph(n_spins: int, graph_seed: int, flags: int = XS_FLAG_GAUGE,
 
 def xs_clause_placement(n_spins: int, graph_seed: int, n_slots: int, flags: int = XS_FLAG_GAUGE | XS_FLAG_BALANCED,
                         set_cap: int = 0):
-    """Host only.  Returns (task [N][4], place [N]) of the clause-word kernel (include/xs.h)."""
-    task = np.zeros((n_spins, 4), np.uint32)
+    """Host only.  Returns (task [rounds * n_slots][4], place [N], barrier_mask) of the clause-word
+    kernel (include/xs.h)."""
+    task = np.zeros((2 * n_spins, 4), np.uint32)
     place = np.zeros(n_spins, np.uint32)
+    nr, bm = C.c_uint32(0), C.c_uint32(0)
     _check(lib().xs_clause_placement(n_spins, int(graph_seed), int(flags), int(set_cap), int(n_slots),
-                                     _ptr(task, C.c_uint32), _ptr(place, C.c_uint32)), "xs_clause_placement")
-    return task, place
+                                     _ptr(task, C.c_uint32), _ptr(place, C.c_uint32), C.byref(nr), C.byref(bm)),
+           "xs_clause_placement")
+    return task[: nr.value * n_slots].copy(), place, int(bm.value)
 
 
 def xs_get_layout(h) -> xs_layout:

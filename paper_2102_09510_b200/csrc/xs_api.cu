@@ -3,6 +3,7 @@
 // method lives here.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstring>
 #include <new>
 
@@ -51,8 +52,10 @@ DevLayout make_layout(const xs_params& p)
     L.off_seed = o;       o = align_up(o + I * 8, 256);
     L.off_det = o;        o = align_up(o + 2 * I * W * 8, 256);
     L.off_nsets = o;      o = align_up(o + I * 4, 256);
-    L.off_crec = o;       o = align_up(o + I * N * sizeof(CRec), 256);
+    L.off_crec = o;       o = align_up(o + I * 2 * N * sizeof(CRec), 256);
     L.off_cplace = o;     o = align_up(o + I * N * 4, 256);
+    L.off_cbar = o;       o = align_up(o + I * 4, 256);
+    L.off_cthr = o;       o = align_up(o + 8, 256);
     L.total = o;
     return L;
 }
@@ -101,6 +104,8 @@ static int finish_create(xs_batch* b, void* dev_ws, size_t ws_bytes, void* strea
     b->d.n_sets = reinterpret_cast<uint32_t*>(ws + b->lay.off_nsets);
     b->d.crec = reinterpret_cast<CRec*>(ws + b->lay.off_crec);
     b->d.cplace = reinterpret_cast<uint32_t*>(ws + b->lay.off_cplace);
+    b->d.cbar = reinterpret_cast<uint32_t*>(ws + b->lay.off_cbar);
+    b->d.cthr = reinterpret_cast<uint32_t*>(ws + b->lay.off_cthr);
 
     // host staging of the tables (pageable; the copies below are synchronous w.r.t. the host)
     std::vector<AdjRec> adj((size_t)I * N);
@@ -353,21 +358,27 @@ int xs_get_graph(const xs_batch* b, uint32_t inst, uint32_t* tri, uint8_t* jbit,
 }
 
 int xs_clause_placement(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uint32_t set_cap,
-                        uint32_t n_slots, uint32_t* task, uint32_t* place)
+                        uint32_t n_slots, uint32_t* task, uint32_t* place, uint32_t* n_rounds,
+                        uint32_t* barrier_mask)
 {
     if (n_spins < 3 || n_spins >= (1u << 24)) return fail(XS_EINVAL, "n_spins out of range");
+    if (n_slots < 2 || n_slots > 256 || (n_slots & 1u)) return fail(XS_EINVAL, "n_slots must be even, 2..256");
     try {
         HostGraph g;
         std::string err;
         if (!build_graph_from_seed(n_spins, graph_seed, (flags & XS_FLAG_GAUGE) != 0, set_cap,
                                    (flags & XS_FLAG_BALANCED) != 0, g, err))
             return fail(XS_EINVAL, err);
-        std::vector<CRec> crec(n_spins);
+        const uint32_t rounds = std::max(4u, clause_rounds(g, n_slots));
+        std::vector<CRec> crec(2ull * n_spins, CRec{0u, 0u, 0u, 0xFFFFFFFFu});
         std::vector<uint32_t> cplace(n_spins);
-        if (!clause_placement(g, n_slots, crec.data(), cplace.data()))
-            return fail(XS_EINVAL, "instance not eligible for the clause-word kernel or no placement found");
-        if (task) std::memcpy(task, crec.data(), (size_t)n_spins * sizeof(CRec));
+        uint32_t bm = 0, mode = 0;
+        if (!clause_placement(g, n_slots, rounds, crec.data(), cplace.data(), &bm, &mode))
+            return fail(XS_EINVAL, "update order does not fit the clause-word kernel on this many slots, or no placement found");
+        if (task) std::memcpy(task, crec.data(), (size_t)rounds * n_slots * sizeof(CRec));
         if (place) std::memcpy(place, cplace.data(), (size_t)n_spins * 4);
+        if (n_rounds) *n_rounds = rounds;
+        if (barrier_mask) *barrier_mask = bm;
     } catch (const std::bad_alloc&) {
         return fail(XS_ENOMEM, "host allocation failed");
     }

@@ -49,7 +49,8 @@ struct alignas(16) ClauseRec {
 };
 
 // Task record of the clause-word kernel (xs_sweep_clause.cu): shared-memory row offsets of the
-// three clause rows of the spin at entry set * n_slots + slot, and the spin index (16 bytes).
+// three clause rows of the spin at entry round * n_slots + slot, and the spin index
+// (0xFFFFFFFF: the slot is idle in that round and works on a scratch row) (16 bytes).
 struct alignas(16) CRec {
     uint32_t off0, off1, off2, spin;
 };
@@ -57,7 +58,7 @@ struct alignas(16) CRec {
 // Device workspace carved out of the caller's buffer.
 struct DevLayout {
     size_t off_x = 0, off_first_hit = 0, off_adj = 0, off_clause = 0, off_set_start = 0,
-           off_rec = 0, off_seed = 0, off_det = 0, off_nsets = 0, off_crec = 0, off_cplace = 0, total = 0;
+           off_rec = 0, off_seed = 0, off_det = 0, off_nsets = 0, off_crec = 0, off_cplace = 0, off_cbar = 0, off_cthr = 0, total = 0;
 };
 DevLayout make_layout(const xs_params& p);
 
@@ -71,7 +72,9 @@ struct DevPtrs {
     uint64_t* run_seed;    // [I]
     uint64_t* det;         // [I][W]   scratch: OR of unsatisfied-clause words
     uint32_t* n_sets;      // [I]
-    CRec* crec;            // [I][N]   clause-word kernel: tasks in slot order
+    CRec* crec;            // [I][2N]  clause-word kernel: tasks, entry = round * n_slots + slot
+    uint32_t* cbar;        // [I]      clause-word kernel: bit r = barrier after round r
+    uint32_t* cthr;        // [2]      clause-word kernel: compare constants of the noise threshold
     uint32_t* cplace;      // [I][N]   clause-word kernel: shared-memory row offset of clause t
 };
 
@@ -114,7 +117,9 @@ struct xs_batch {
     uint32_t max_set_size = 0;
     uint32_t clause_state = 0;    // clause-word kernel tables: 0 not built, 1 uploaded, 2 not eligible
     uint32_t clause_slots = 0;    // slots per CTA the uploaded tables were built for
-    uint32_t clause_rounds = 0;   // sets per sweep of those tables (4 or 6)
+    uint32_t clause_rounds = 0;   // rounds per sweep of those tables (4..8)
+    uint64_t clause_thr = ~0ull;  // threshold the uploaded compare constants belong to
+    uint32_t clause_mode = 0;     // kernel MODE the tables allow (xs_sweep_clause.cuh)
     uint64_t sweeps_issued = 0;   // upper bound on any instance's sweep counter (overflow guard)
     xs_geometry req{XS_GEOM_AUTO, 0, 0, 0, 0, 0};   // xs_set_geometry requests (0 / AUTO = rule)
     uint32_t num_sms = 148;       // cudaDevAttrMultiProcessorCount of the device the batch lives on
@@ -136,7 +141,9 @@ uint32_t static_rounds(const xs_batch& b, uint32_t T, uint32_t CW, uint32_t thre
 uint32_t static_smem_bytes(uint32_t N, uint32_t T);
 int launch_sweep_static(const xs_batch& b, uint32_t n_sweeps, void* stream);
 // clause-word variant (xs_sweep_clause.cu)
-bool clause_placement(const HostGraph& g, uint32_t n_slots, CRec* crec, uint32_t* cplace);
+uint32_t clause_rounds(const HostGraph& g, uint32_t n_slots);
+bool clause_placement(const HostGraph& g, uint32_t n_slots, uint32_t n_rounds, CRec* crec,
+                      uint32_t* cplace, uint32_t* bar_mask, uint32_t* mode);
 int clause_prepare(xs_batch& b, void* stream);
 int launch_sweep_clause(const xs_batch& b, uint32_t n_sweeps, void* stream);
 }  // namespace xs

@@ -74,42 +74,63 @@ def test_balanced_sets_match_oracle(N, seed, cap):
         assert np.array_equal(order, g.order)
 
 
-@pytest.mark.parametrize("N,seed,n_slots", [(256, 2, 64), (128, 100, 32), (512, 101, 128), (512, 355, 128),
-                                            (192, 7, 32), (384, 8, 64), (768, 9, 128), (128, 128004, 32),
-                                            (64, 5, 16)])
-def test_clause_placement_is_conflict_free_and_complete(N, seed, n_slots):
+@pytest.mark.parametrize("N,seed,n_slots,balanced,cap", [
+    (256, 2, 64, True, 0), (128, 100, 32, True, 0), (512, 101, 128, True, 0), (512, 355, 128, True, 0),
+    (192, 7, 32, True, 0), (384, 8, 64, True, 0), (768, 9, 128, True, 0), (128, 128004, 32, True, 0),
+    (1024, 1024000, 128, True, 0),     # 4 sets of 256 on 128 slots: 8 rounds, barrier after every second
+    (160, 3, 32, True, 0), (224, 4, 32, True, 0), (320, 5, 64, True, 0),     # 5 / 7 / 5 sets
+    (256, 2, 64, False, 0), (512, 100, 128, False, 0), (128, 9, 32, False, 0),  # greedy, ragged sets
+    (100, 6, 32, True, 25), (200, 11, 64, False, 0)])
+def test_clause_placement_is_conflict_free_and_complete(N, seed, n_slots, balanced, cap):
     """Placement tables of the clause-word kernel (include/xs.h), checked straight
-    from the triplets: every set's entries are exactly the set's spins (L277: any order inside a
-    set is valid), an entry's three rows are the three interactions the spin enters (L67), and
-    the two slots of a shared-memory phase touch opposite halves of their 128-byte lines."""
-    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_BALANCED
-    tri, jbit, order, ss, att = xs.xs_generate_graph(N, seed, fl, 0)
-    assert len(ss) in (4, 6) and (ss == n_slots).all()
-    task, place = xs.xs_clause_placement(N, seed, n_slots, fl, 0)
+    from the triplets: the entries of a set's rounds are exactly the set's spins (L277: any order
+    inside a set is valid), an entry's three rows are the three interactions the spin enters (L67),
+    idle slots stay on their scratch line, and the two slots of a shared-memory phase touch
+    opposite halves of their 128-byte lines."""
+    fl = xs.XS_FLAG_GAUGE | (xs.XS_FLAG_BALANCED if balanced else 0)
+    tri, jbit, order, ss, att = xs.xs_generate_graph(N, seed, fl, cap)
+    task, place, bar = xs.xs_clause_placement(N, seed, n_slots, fl, cap)
+    n_rounds = len(task) // n_slots
+    assert 4 <= n_rounds <= 8 and n_rounds * n_slots <= 2 * N
     t = np.arange(N, dtype=np.uint32)
     assert np.array_equal(place & ~np.uint32(64), t << 7)                 # own line, lower or upper half
     clauses_of = [[] for _ in range(N)]
     for c, (i, j, k) in enumerate(tri.tolist()):
         for v in (i, j, k):
             clauses_of[v].append(c)
-    for s in range(len(ss)):
-        ent = task[s * n_slots:(s + 1) * n_slots]
-        assert sorted(ent[:, 3].tolist()) == sorted(order[s * n_slots:(s + 1) * n_slots].tolist())
-        for e in ent:
+    IDLE = 0xFFFFFFFF
+    r0, p0, want_bar = 0, 0, 0
+    for sz in ss.tolist():
+        nr = -(-sz // n_slots)
+        ent = task[r0 * n_slots:(r0 + nr) * n_slots]
+        spins = ent[ent[:, 3] != IDLE, 3]
+        assert sorted(spins.tolist()) == sorted(order[p0:p0 + sz].tolist())
+        r0, p0 = r0 + nr, p0 + sz
+        want_bar |= 1 << (r0 - 1)
+    assert bar == want_bar
+    assert (task[r0 * n_slots:, 3] == IDLE).all()                         # padding rounds are idle
+    for e_i, e in enumerate(task):
+        if e[3] != IDLE:
             assert sorted((e[:3] >> 7).tolist()) == sorted(clauses_of[int(e[3])])
             assert np.array_equal(e[:3], place[e[:3] >> 7])
-        half = (ent[:, :3] >> 6) & 1
-        assert ((half[0::2] ^ half[1::2]) == 1).all()
+        else:
+            assert ((e[:3] >> 7) == N + (e_i % n_slots) // 2).all()       # scratch line of the slot pair
+    half = (task[:, :3] >> 6) & 1
+    assert ((half[0::2] ^ half[1::2]) == 1).all()
+    if balanced and cap == 0 and N % (n_slots * 4) == 0 and len(ss) * n_slots == N:
+        assert (task[:, 3] != IDLE).all()                                 # full sets: no idle slot
     # deterministic
-    task2, place2 = xs.xs_clause_placement(N, seed, n_slots, fl, 0)
-    assert np.array_equal(task, task2) and np.array_equal(place, place2)
+    task2, place2, bar2 = xs.xs_clause_placement(N, seed, n_slots, fl, cap)
+    assert np.array_equal(task, task2) and np.array_equal(place, place2) and bar == bar2
 
 
-def test_clause_placement_rejects_ineligible_shapes():
-    with pytest.raises(xs.XsError):                     # greedy sets: ragged
-        xs.xs_clause_placement(256, 2, 64, xs.XS_FLAG_GAUGE, 0)
-    with pytest.raises(xs.XsError):                     # sets of 64 on 32 slots
-        xs.xs_clause_placement(256, 2, 32)
+def test_clause_placement_rejects_orders_that_do_not_fit():
+    with pytest.raises(xs.XsError):                     # sets of 64 on 16 slots: 16 rounds
+        xs.xs_clause_placement(256, 2, 16)
+    with pytest.raises(xs.XsError):                     # cap-32 order (PAPER.md L279): 17+ sets
+        xs.xs_clause_placement(512, 2, 32, xs.XS_FLAG_GAUGE, 32)
+    with pytest.raises(xs.XsError):                     # odd slot count
+        xs.xs_clause_placement(256, 2, 63)
 
 
 def test_workspace_bytes_and_param_errors():
