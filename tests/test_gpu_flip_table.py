@@ -86,11 +86,12 @@ def test_back_to_quasi_greedy_table_uses_fast_kernel():
     import paper_2102_09510_b200 as xs
     N, W = 64, 8
     b = xs.Batch(N, W, [5], [6], flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP)
-    assert b.layout().variant == 1
+    fast = b.layout().variant
+    assert fast in (1, 2)
     b.set_flip_table(metropolis(1.0))
     assert b.layout().variant == 0
     b.set_flip_table([0, 200000000, TWO32, TWO32])       # quasi-greedy form with another w1
-    assert b.layout().variant == 1
+    assert b.layout().variant == fast
     o = OracleRun(N, W, 5, 6, no_skip=True, thr=200000000)
     b.run_sweeps(30)
     o.run_sweeps(30)

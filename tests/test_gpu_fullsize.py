@@ -35,13 +35,14 @@ def _check_words(b, o, inst=0):
 @pytest.mark.parametrize("balanced", [True, False])
 def test_config2_full_size_sampled_words(balanced):
     """configs[1]: N=256, graph seed 2, 2^16 clones; bench.py's launch configuration (balanced
-    sets of 64, clause-word kernel, T=8) and the greedy-order variant (`--workload config2_greedy`)."""
+    sets of 64, clause-word kernel, T=8) and the greedy-order variant (`--workload config2_greedy`:
+    6 ragged sets on 64 slots, same kernel with idle slots)."""
     import paper_2102_09510_b200 as xs
     N, W = 256, 1024
     fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_BALANCED if balanced else 0)
     b = xs.Batch(N, W, [2], [2], set_cap=64 if balanced else 0, flags=fl)
     lay = b.layout()
-    assert (lay.regime, lay.variant, lay.tile_words, lay.ctas) == (0, 2 if balanced else 1, 8, 128)
+    assert (lay.regime, lay.variant, lay.tile_words, lay.ctas) == (0, 2, 8, 128)
     assert lay.n_sets_max == (4 if balanced else 6)
     words = [0, 7, 8, 517, 1023]          # first/last lane of a tile, tile boundaries, last tile
     o = OracleRun(N, W, 2, 2, set_cap=64 if balanced else 0, no_skip=True, words=words,
@@ -62,13 +63,13 @@ def test_config2_full_size_sampled_words(balanced):
 def test_config3_shape_sampled_instances_and_words(balanced):
     """configs[2] shape: N=512, W=64 per instance, 160 instances so that every SM gets a tile.
     balanced (bench.py --workload config3): 4 sets of 128 -> clause-word kernel, T=8, 512 threads;
-    greedy (config3_greedy): generic kernel, T=16 -- the geometries the 256-instance runs use."""
+    greedy (config3_greedy): same kernel, ragged sets on 128 slots -- the geometries the 256-instance runs use."""
     import paper_2102_09510_b200 as xs
     N, W, I = 512, 64, 160
     seeds = list(range(100, 100 + I))
     b = xs.Batch(N, W, seeds, seeds, flags=xs.XS_FLAG_GAUGE | (xs.XS_FLAG_BALANCED if balanced else 0))
     lay = b.layout()
-    assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == ((0, 2, 8, 512) if balanced else (0, 0, 16, 512))
+    assert (lay.regime, lay.variant, lay.tile_words, lay.threads) == (0, 2, 8, 512)
     checks = {0: [0, 15, 16], 77: [33, 63], 159: [48]}
     oracles = {i: OracleRun(N, W, seeds[i], seeds[i], words=ws, balanced=balanced) for i, ws in checks.items()}
     for n in (70, 563):                   # 633 sweeps: two full 256-sweep detection batches + a remainder
@@ -82,7 +83,7 @@ def test_config3_shape_sampled_instances_and_words(balanced):
 
 
 @pytest.mark.parametrize("N,threads,tile", [(128, 128, 8), (192, 128, 8), (256, 256, 8), (384, 256, 8),
-                                            (768, 512, 8), (1024, 1024, 8)])
+                                            (768, 512, 8), (1024, 512, 8)])
 def test_config4_shapes_balanced_static_geometry(N, threads, tile):
     """configs[3] shapes that run on the static kernel in bench.py (--workload config4_N): 160
     instances of W = 8 give one tile per SM and more; sampled instances, all words."""
