@@ -52,7 +52,7 @@ DevLayout make_layout(const xs_params& p)
     L.off_seed = o;       o = align_up(o + I * 8, 256);
     L.off_det = o;        o = align_up(o + 2 * I * W * 8, 256);
     L.off_nsets = o;      o = align_up(o + I * 4, 256);
-    L.off_crec = o;       o = align_up(o + I * 2 * N * sizeof(CRec), 256);
+    L.off_crec = o;       o = align_up(o + I * (size_t)crec_entries(p) * sizeof(CRec), 256);
     L.off_cplace = o;     o = align_up(o + I * N * 4, 256);
     L.off_cbar = o;       o = align_up(o + I * 4, 256);
     L.off_cthr = o;       o = align_up(o + 8, 256);
@@ -160,6 +160,7 @@ static int finish_create(xs_batch* b, void* dev_ws, size_t ws_bytes, void* strea
     std::string err;
     if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
     if (int e = clause_prepare(*b, stream)) return cuda_fail(e, "clause tables");
+    if (int e = warp_prepare(*b, stream)) return cuda_fail(e, "latency kernel tables");
     if (int e = launch_init(*b, stream)) return cuda_fail(e, "init kernel");
     if (int e = launch_mark(*b, true, stream)) return cuda_fail(e, "mark kernel");
     if (int e = launch_finalize(*b, 0, stream)) return cuda_fail(e, "finalize kernel");
@@ -266,6 +267,7 @@ int xs_set_flip_table(xs_batch* b, const uint64_t* thr4, void* cuda_stream)
     std::string err;
     if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
     if (int e = clause_prepare(*b, cuda_stream)) return cuda_fail(e, "clause tables");
+    if (int e = warp_prepare(*b, cuda_stream)) return cuda_fail(e, "latency kernel tables");
     return XS_OK;
 }
 
@@ -290,6 +292,7 @@ int xs_set_geometry(xs_batch* b, const xs_geometry* g, void* cuda_stream)
         return fail(XS_EINVAL, err);
     }
     if (int e = clause_prepare(*b, cuda_stream)) return cuda_fail(e, "clause tables");
+    if (int e = warp_prepare(*b, cuda_stream)) return cuda_fail(e, "latency kernel tables");
     return XS_OK;
 }
 

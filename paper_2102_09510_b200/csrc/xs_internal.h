@@ -61,6 +61,13 @@ struct DevLayout {
            off_rec = 0, off_seed = 0, off_det = 0, off_nsets = 0, off_crec = 0, off_cplace = 0, off_cbar = 0, off_cthr = 0, total = 0;
 };
 DevLayout make_layout(const xs_params& p);
+// Task-table entries per instance (CRec crec[I][entries]): 2 N, and at least 256 for batches of up
+// to 1024 small instances so that the latency kernel's 16-slot passes always fit.
+inline uint32_t crec_entries(const xs_params& p)
+{
+    const uint32_t e = 2u * p.n_spins;
+    return (e < 256u && p.n_instances <= 1024u) ? 256u : e;
+}
 
 struct DevPtrs {
     uint64_t* x;           // [I][N][W]
@@ -119,7 +126,8 @@ struct xs_batch {
     uint32_t clause_slots = 0;    // slots per CTA the uploaded tables were built for
     uint32_t clause_rounds = 0;   // rounds per sweep of those tables (4..8)
     uint64_t clause_thr = ~0ull;  // threshold the uploaded compare constants belong to
-    uint32_t clause_mode = 0;     // kernel MODE the tables allow (xs_sweep_clause.cuh)
+    uint32_t clause_mode = 0;
+    uint32_t warp_passes = 0;     // latency kernel: passes per sweep of the uploaded tables (0 = none)     // kernel MODE the tables allow (xs_sweep_clause.cuh)
     uint64_t sweeps_issued = 0;   // upper bound on any instance's sweep counter (overflow guard)
     xs_geometry req{XS_GEOM_AUTO, 0, 0, 0, 0, 0};   // xs_set_geometry requests (0 / AUTO = rule)
     uint32_t num_sms = 148;       // cudaDevAttrMultiProcessorCount of the device the batch lives on
@@ -146,4 +154,7 @@ bool clause_placement(const HostGraph& g, uint32_t n_slots, uint32_t n_rounds, C
                       uint32_t* cplace, uint32_t* bar_mask, uint32_t* mode);
 int clause_prepare(xs_batch& b, void* stream);
 int launch_sweep_clause(const xs_batch& b, uint32_t n_sweeps, void* stream);
+// latency kernel (xs_sweep_warp.cu)
+int warp_prepare(xs_batch& b, void* stream);
+int launch_sweep_warp(const xs_batch& b, uint32_t n_sweeps, void* stream);
 }  // namespace xs

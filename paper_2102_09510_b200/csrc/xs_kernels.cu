@@ -919,6 +919,7 @@ int launch_sweeps(const xs_batch& b, uint32_t n_sweeps, void* stream)
     const TileGeom& g = b.geom;
     cudaStream_t st = (cudaStream_t)stream;
     if (n_sweeps == 0) return 0;
+    if (g.regime == 0 && g.variant == 3) return launch_sweep_warp(b, n_sweeps, stream);
     if (g.regime == 0 && g.variant == 2) return launch_sweep_clause(b, n_sweeps, stream);
     if (g.regime == 0 && g.variant == 1) return launch_sweep_static(b, n_sweeps, stream);
     if (g.regime == 0) {

@@ -27,7 +27,8 @@
 //
 // Noise (a-6): one Philox4x32-10 call yields the numbers of 4 consecutive words of a spin for one
 // sweep.  The two lanes that share a word group each compute the call of one sweep of a two-sweep
-// period and exchange the threshold bytes by shuffles.  The 10 round keys are CTA-uniform: the
+// period and exchange the threshold bytes by shuffles (one register per round; even and odd
+// rounds renew it in alternate sweeps, so every round carries half a call).  The 10 round keys are CTA-uniform: the
 // run seed comes from the kernel parameters (constant bank), so the key schedule lives in uniform
 // registers and costs no vector ALU work.  The comparison u < thr runs on the FMA pipe: the carry
 // of u + (2^32 - thr) is the high word of a 64-bit multiply-add, and the four carries are packed
@@ -58,9 +59,12 @@ struct ClauseArgs {
     DevPtrs d;
     uint32_t N, W, n_sweeps, flags, batch;
     uint32_t n_slots;        // slots per CTA = threads / 4
+    uint32_t ent;            // task-table entries per instance (crec_entries)
     uint32_t inst0;          // first instance of this launch
     uint32_t off_misc;       // byte offset of det32 / known32 / flag in dynamic shared memory
+    uint32_t thr;            // noise threshold: a k = 1 spin flips iff u < thr
     uint32_t one;            // the multiplier 1, as data, so that the compare stays a multiply-add
+    uint32_t zero;           // the multiplier 0, as data: ties the last store of a round to its Philox call
     uint64_t seed[CL_MAXI];  // run seeds of instances inst0 .. (constant bank -> uniform registers)
 };
 
@@ -102,6 +106,11 @@ constexpr int LUT_OR_ANDN = 0xF4;   // a | (b & ~c)
 template <int R, int MAXTHREADS, int MINB, int MODE>
 __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_constant__ ClauseArgs A)
 {
+    // One CTA per SM with few warps (fewer tiles than SMs, e.g. BASELINE.json configs[1]): the
+    // kernel is bound by the dependent chain of a round, not by a pipe.  Measured (DESIGN.md
+    // section 7): the multiply-add compare and the store-address tie of the noise cost 3 % there
+    // and gain 10 % on the dense shapes, so the two launch classes take different forms.
+    constexpr bool SPARSE = (MINB == 1 && MAXTHREADS <= 256);
     extern __shared__ __align__(128) unsigned char smem[];
     const uint32_t N = A.N, W = A.W;
     const uint32_t tiles = W / CL_T;
@@ -134,7 +143,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     uint32_t rm[R];           // threshold bytes of the current two-sweep noise period
     uint32_t act = 0, wact = 0, bar = 0;
     {
-        const uint4* cr = reinterpret_cast<const uint4*>(A.d.crec + (size_t)inst * 2u * N);
+        const uint4* cr = reinterpret_cast<const uint4*>(A.d.crec + (size_t)inst * A.ent);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const uint4 v = cr[r * n_slots + slot];
@@ -200,41 +209,67 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     const uint2 ta = *reinterpret_cast<const uint2*>(A.d.cthr);
     const uint64_t addend = ((uint64_t)ta.y << 32) | ta.x;
     const uint32_t one = A.one;
+    // Noise periods: round r works in periods of two sweeps with phase phi = r & 1: period k of round
+    // r covers sweeps 2k - phi and 2k - phi + 1, so that half of the rounds renew their threshold
+    // bytes in even sweeps and the other half in odd sweeps (every round of every sweep carries
+    // the same work: 7 logic operations per 32 clones + half a Philox call).
     // bytes of the result: byte 2h + c = 0xFF iff word c of this lane does NOT flip k = 1 spins in
-    // sweep h of period q (u >= thr)
-    auto noise_call = [&](int r, uint32_t q) -> uint32_t {
+    // sweep h of the period (u >= thr)
+    auto noise_call = [&](int r, uint32_t k, uint32_t& own) -> uint32_t {
         uint32_t o[4];
-        philox4x32_10(spin[r], grp, 2u * q + jl, TAG_SWEEP, k0, k1, o);
+        philox4x32_10(spin[r], grp, 2u * k - (uint32_t)(r & 1) + jl, TAG_SWEEP, k0, k1, o);
         uint32_t v = 0;
+        if (SPARSE) {
+            // plain compares: the shortest dependent chain (set-predicate, select, OR)
+            const uint32_t thr = A.thr;
+            v = (o[0] >= thr ? 0xFFu : 0u) | (o[1] >= thr ? 0xFF00u : 0u) |
+                (o[2] >= thr ? 0xFF0000u : 0u) | (o[3] >= thr ? 0xFF000000u : 0u);
+        } else {
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const uint32_t ge = (uint32_t)(cl_mad_wide(o[i], one, addend) >> 32);   // 1 iff o[i] >= thr
-            v = cl_mad_lo(ge, 0xFFu << (8 * i), v);
+            for (int i = 0; i < 4; ++i) {
+                const uint32_t ge = (uint32_t)(cl_mad_wide(o[i], one, addend) >> 32);   // 1 iff o[i] >= thr
+                v = cl_mad_lo(ge, 0xFFu << (8 * i), v);
+            }
         }
+        own = v;
         const uint32_t s0 = __shfl_sync(0xFFFFFFFFu, v, lane_base);
         const uint32_t s1 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 1);
         return cl_prmt(s0, s1, sub_sel);
     };
-    auto produce_all = [&](uint32_t q) {
+    // threshold bytes of the periods that contain sweep t
+    auto produce_all = [&](uint32_t t) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) rm[r] = noise_call(r, q);
+        for (int r = 0; r < R; ++r) {
+            uint32_t own;
+            rm[r] = noise_call(r, (t + (uint32_t)(r & 1)) >> 1, own);
+        }
     };
 
-    // ---- one sweep (a-4..a-8); h = index of the sweep inside the noise period.  In the second
-    // sweep of a period every round replaces its threshold bytes by those of period qn right after
-    // their last use; the Philox chain sits in the latency shadow of the round's loads. ----------
-    auto sweep = [&](auto hc, uint32_t qn) {
+    // ---- sweep t (a-4..a-8); h = t & 1.  A round in the second sweep of its period replaces its
+    // threshold bytes by those of the next period right after their last use; the Philox chain sits
+    // in the latency shadow of the round's loads. ------------------------------------------------
+    auto sweep = [&](auto hc, uint32_t t) {
         constexpr uint32_t h = decltype(hc)::value;
-        constexpr uint32_t sel0 = 0x8888u + 0x1111u * (2u * h);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             if (MODE != 0 || ((wact >> r) & 1u)) {
+                const uint32_t hp = h ^ (uint32_t)(r & 1);          // sweep index inside the round's period
+                const uint32_t sel0 = 0x8888u + 0x1111u * (2u * hp);
                 uint32_t c0[CL_H], c1[CL_H], c2[CL_H];
                 cl_lds4(ca[r][0], c0); cl_lds4(ca[r][1], c1); cl_lds4(ca[r][2], c2);
                 uint32_t nf[2];
                 nf[0] = cl_prmt(rm[r], 0u, sel0);
                 nf[1] = cl_prmt(rm[r], 0u, sel0 + 0x1111u);
-                if (h == 1) rm[r] = noise_call(r, qn);
+                // The address of the round's last store is made to depend (times zero) on the call's
+                // result: the instruction scheduler then treats the Philox chain as the critical path
+                // of the round and issues it first, interleaved with the update, in the shadow of
+                // the loads, instead of leaving the loads' latency exposed and the chain for later.
+                uint32_t a2 = ca[r][2];
+                if (hp == 1) {
+                    uint32_t own;
+                    rm[r] = noise_call(r, ((t + (uint32_t)(r & 1)) >> 1) + 1u, own);
+                    if (!SPARSE) a2 = cl_mad_lo(own, A.zero, a2);
+                }
 #pragma unroll
                 for (int c = 0; c < CL_H; ++c) {
                     const uint32_t M = lop3<LUT_MAJ>(c0[c], c1[c], c2[c]);     // k >= 2
@@ -243,7 +278,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
                     c0[c] ^= f; c1[c] ^= f; c2[c] ^= f;
                     x[r][c] ^= f;
                 }
-                cl_sts4(ca[r][0], c0); cl_sts4(ca[r][1], c1); cl_sts4(ca[r][2], c2);
+                cl_sts4(ca[r][0], c0); cl_sts4(ca[r][1], c1); cl_sts4(a2, c2);
             }
             if (MODE == 1 || (MODE == 2 && (r & 1)) || (MODE == 0 && ((bar >> r) & 1u)))
                 __syncthreads();                                              // a-8
@@ -289,20 +324,20 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
         };
         uint32_t t = t0 + 1;
         const uint32_t t_last = t0 + n;
-        produce_all(t >> 1);                         // noise of the period that contains sweep t
+        produce_all(t);
         if (t & 1u) {
-            sweep(std::integral_constant<uint32_t, 1>{}, (t >> 1) + 1u);
+            sweep(std::integral_constant<uint32_t, 1>{}, t);
             post(t);
             ++t;
         }
         for (; t < t_last; t += 2) {
-            sweep(std::integral_constant<uint32_t, 0>{}, 0u);
+            sweep(std::integral_constant<uint32_t, 0>{}, t);
             post(t);
-            sweep(std::integral_constant<uint32_t, 1>{}, (t >> 1) + 1u);
+            sweep(std::integral_constant<uint32_t, 1>{}, t + 1);
             post(t + 1);
         }
         if (t == t_last) {
-            sweep(std::integral_constant<uint32_t, 0>{}, 0u);
+            sweep(std::integral_constant<uint32_t, 0>{}, t);
             post(t);
         }
     };

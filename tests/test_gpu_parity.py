@@ -146,6 +146,7 @@ def test_config1_until_solved_matches_oracle_and_survey_hint(golden):
     hint = dict(line.split(None, 1) for line in open(golden("config1_survey_hint.txt"))
                 if line.strip() and not line.startswith("#"))
     b = xs.Batch(64, 1, [1], [1])
+    assert b.layout().variant == 3            # the latency kernel (one consumer warp + noise producers)
     o = OracleRun(64, 1, 1, 1)
     for _ in range(1000):
         b.run_sweeps(100)
@@ -162,6 +163,61 @@ def test_config1_until_solved_matches_oracle_and_survey_hint(golden):
     o.run_sweeps(100)
     assert np.array_equal(b.spins_numpy(), x0)
     _compare(b, [o], "config 1 after solve")
+    b.close()
+
+
+@pytest.mark.parametrize("N,W,I,cap,balanced", [
+    (64, 1, 1, 0, False),      # configs[0] shape
+    (64, 4, 3, 0, False),      # four consumer warps, three instances
+    (18, 2, 2, 0, False),      # tiny: clones solve all the time -> replay of the 32-sweep chunk
+    (128, 1, 5, 0, True),      # 4 balanced sets of 32 = 8 passes of 16
+    (200, 3, 1, 0, False),     # 16 passes (second instantiation)
+    (96, 2, 1, 16, False),     # capped sets
+])
+def test_latency_kernel_parity(N, W, I, cap, balanced):
+    """k_sweep_warp (layout variant 3): few instances with W <= 4 words; lanes <-> spins of the set,
+    noise produced ahead by the producer warps.  Calls of 1, 31, 33 and 70 sweeps cross the 32-sweep
+    noise chunks at odd offsets; resume must be exact."""
+    xs = _xs()
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | (xs.XS_FLAG_BALANCED if balanced else 0)
+    gs = [N + 2 + i for i in range(I)]
+    rs = [5 * N + i for i in range(I)]
+    b = xs.Batch(N, W, gs, rs, set_cap=cap, flags=fl, geometry=dict(variant=3))
+    lay = b.layout()
+    assert (lay.regime, lay.variant, lay.tile_words, lay.ctas) == (0, 3, W, I), (lay.variant, lay.tile_words)
+    os_ = [OracleRun(N, W, g, r, set_cap=cap, no_skip=True, balanced=balanced) for g, r in zip(gs, rs)]
+    for n in (1, 31, 33, 70):
+        b.run_sweeps(n)
+        for o in os_:
+            o.run_sweeps(n)
+        _compare(b, os_, f"latency kernel N={N} W={W} after {n}")
+    if N == 18:
+        assert (os_[0].first_hit != NO_HIT).sum() > 20
+    b.close()
+
+
+def test_latency_kernel_stop_rule_and_geometry_requests():
+    """Solved instances are skipped by the latency kernel too; malformed geometry requests are
+    refused; a request the shape cannot satisfy falls back to the rule."""
+    xs = _xs()
+    N, W = 32, 1
+    gseeds, rseeds = list(range(3, 11)), list(range(13, 21))
+    b = xs.Batch(N, W, gseeds, rseeds, set_cap=16, flags=xs.XS_FLAG_GAUGE, geometry=dict(variant=3))
+    assert b.layout().variant == 3
+    os_ = [OracleRun(N, W, g, r, set_cap=16) for g, r in zip(gseeds, rseeds)]
+    for _ in range(10):
+        b.run_sweeps(20)
+        for o in os_:
+            o.run_sweeps(20)
+        _compare(b, os_, "latency kernel stop rule")
+    assert len({o.sweeps_done for o in os_}) > 1
+    for bad in (dict(tile_words=3), dict(threads=100), dict(words_per_lane=3), dict(variant=9)):
+        with pytest.raises(xs.XsError) as ei:
+            b.set_geometry(**bad)
+        assert ei.value.code == -1
+    b.set_geometry(variant=2)                  # W = 1: the clause-word kernel cannot take it
+    assert b.layout().variant in (0, 1)
+    b.set_geometry()                           # back to the rule
     b.close()
 
 
