@@ -192,7 +192,7 @@ int clause_prepare(xs_batch& b, void* stream)
     if (g.regime != 0 || b.ft.general || b.ft.per_clone || (b.p.flags & XS_FLAG_STREAMING)) return 0;
     if (rq.tile_words && rq.tile_words != CL_T) return 0;
     const uint32_t N = b.p.n_spins, I = b.p.n_instances, W = b.p.n_words;
-    if (W % CL_T || N < 64u) return 0;
+    if (W % CL_T || N < 64u || N >= (1u << 14)) return 0;
     // CTA size: the one that needs the fewest rounds per sweep (ties: the smaller CTA)
     uint32_t threads = 0, rounds = ~0u;
     for (uint32_t thr : {128u, 256u, 512u}) {

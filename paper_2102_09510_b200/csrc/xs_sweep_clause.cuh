@@ -138,9 +138,18 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
 
     // ---- static task list: this thread's spin of round r = entry r * n_slots + slot -----------
     uint32_t ca[R][3];        // shared addresses of the spin's three clause rows
-    uint32_t spin[R];
     uint32_t x[R][CL_H];      // the spin's words: registers only
-    uint32_t rm[R];           // threshold bytes of the current two-sweep noise period
+    // threshold bytes of the current two-sweep noise period.  Only bit 7 of each byte is looked at
+    // (sign-replicating PRMT); with 7 or 8 rounds the spin index rides in bits 0-6 of bytes 0 and 1
+    // (N < 2^14): one register per round less, which keeps the 8-round list of N = 1024 free of
+    // spills under the 128-register cap.  (Measured: the unpacking costs 6 % with 4 rounds, where
+    // there is room, and gains 3 % with 8.)
+    constexpr bool PACK = (R >= 7);
+    uint32_t rm[R];
+    uint32_t spin[PACK ? 1 : R];
+    auto spin_of = [&](int r) -> uint32_t {
+        return PACK ? ((rm[r] & 0x7Fu) | ((rm[r] >> 1) & 0x3F80u)) : spin[PACK ? 0 : r];
+    };
     uint32_t act = 0, wact = 0, bar = 0;
     {
         const uint4* cr = reinterpret_cast<const uint4*>(A.d.crec + (size_t)inst * A.ent);
@@ -150,8 +159,12 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
             ca[r][0] = lane_off + v.x;
             ca[r][1] = lane_off + v.y;
             ca[r][2] = lane_off + v.z;
-            spin[r] = v.w;
-            rm[r] = 0;
+            if (PACK) {
+                rm[r] = (v.w & 0x7Fu) | ((v.w & 0x3F80u) << 1);
+            } else {
+                rm[r] = 0;
+                spin[PACK ? 0 : r] = v.w;
+            }
             if (MODE == 0) {
                 const bool a = v.w != CL_IDLE;
                 if (a) act |= 1u << r;
@@ -175,7 +188,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             if (MODE != 0 || ((act >> r) & 1u)) {
-                const uint4 v = *reinterpret_cast<const uint4*>(xg + (size_t)spin[r] * W + 2u * j);
+                const uint4 v = *reinterpret_cast<const uint4*>(xg + (size_t)spin_of(r) * W + 2u * j);
                 x[r][0] = v.x; x[r][1] = v.y; x[r][2] = v.z; x[r][3] = v.w;
             } else {
                 x[r][0] = x[r][1] = x[r][2] = x[r][3] = 0u;
@@ -187,7 +200,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
 #pragma unroll
         for (int r = 0; r < R; ++r)
             if (MODE != 0 || ((act >> r) & 1u))
-                *reinterpret_cast<uint4*>(xg + (size_t)spin[r] * W + 2u * j) =
+                *reinterpret_cast<uint4*>(xg + (size_t)spin_of(r) * W + 2u * j) =
                     make_uint4(x[r][0], x[r][1], x[r][2], x[r][3]);
     };
     load_state();
@@ -217,7 +230,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     // sweep h of the period (u >= thr)
     auto noise_call = [&](int r, uint32_t k, uint32_t& own) -> uint32_t {
         uint32_t o[4];
-        philox4x32_10(spin[r], grp, 2u * k - (uint32_t)(r & 1) + jl, TAG_SWEEP, k0, k1, o);
+        philox4x32_10(spin_of(r), grp, 2u * k - (uint32_t)(r & 1) + jl, TAG_SWEEP, k0, k1, o);
         uint32_t v = 0;
         if (SPARSE) {
             // plain compares: the shortest dependent chain (set-predicate, select, OR)
@@ -234,7 +247,9 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
         own = v;
         const uint32_t s0 = __shfl_sync(0xFFFFFFFFu, v, lane_base);
         const uint32_t s1 = __shfl_sync(0xFFFFFFFFu, v, lane_base + 1);
-        return cl_prmt(s0, s1, sub_sel);
+        const uint32_t nb = cl_prmt(s0, s1, sub_sel);
+        // PACK: new threshold bits (bit 7 of every byte), the spin index bits stay
+        return PACK ? lop3<0xE4>(nb, rm[r], 0x80808080u) : nb;             // c ? a : b
     };
     // threshold bytes of the periods that contain sweep t
     auto produce_all = [&](uint32_t t) {
