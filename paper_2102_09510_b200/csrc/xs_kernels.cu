@@ -55,16 +55,14 @@ __global__ void k_init(DevPtrs d, uint32_t N, uint32_t W, uint32_t I)
 // unsatisfied clause <=> E_c > -N (L41: each of the N terms is >= -1).
 // grid = (clause chunks, I); a thread owns words w = tid, tid + blockDim, ...
 // ------------------------------------------------------------------------------------------
-constexpr uint32_t DET_CHUNK = 64;
-
-__global__ void k_unsat_or(DevPtrs d, uint32_t N, uint32_t W, uint64_t* det)
+__global__ void k_unsat_or(DevPtrs d, uint32_t N, uint32_t W, uint32_t chunk, uint64_t* det)
 {
     const uint32_t inst = blockIdx.y;
-    const uint32_t c0 = blockIdx.x * DET_CHUNK;
-    const uint32_t c1 = min(c0 + DET_CHUNK, N);
+    const uint32_t c0 = blockIdx.x * chunk;
+    const uint32_t c1 = min(c0 + chunk, N);
     const ClauseRec* cl = d.clause + (size_t)inst * N;
     const uint64_t* x = d.x + (size_t)inst * N * W;
-    for (uint32_t w = threadIdx.x; w < W; w += blockDim.x) {
+    for (uint32_t w = blockIdx.z * blockDim.x + threadIdx.x; w < W; w += gridDim.z * blockDim.x) {
         uint64_t acc = 0;
         for (uint32_t c = c0; c < c1; ++c) {
             const ClauseRec r = cl[c];
@@ -173,17 +171,24 @@ __global__ void __launch_bounds__(EN_THREADS) k_energy_acc(DevPtrs d, uint32_t N
 // a-11 / a-12: per-instance record.  TTS = min_c first_hit (L111); smallest clone on ties.
 // One CTA per instance.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_finalize(DevPtrs d, uint32_t W, uint32_t n_sweeps,
-                                                  uint32_t flags)
+constexpr uint32_t FIN_THREADS = 1024;
+
+__global__ void __launch_bounds__(FIN_THREADS) k_finalize(DevPtrs d, uint32_t W, uint32_t n_sweeps,
+                                                          uint32_t flags)
 {
-    __shared__ unsigned long long best[8];
+    __shared__ unsigned long long best[FIN_THREADS / 32];
     const uint32_t inst = blockIdx.x;
-    const uint32_t C = 64 * W;
-    const uint32_t* fh = d.first_hit + (size_t)inst * C;
+    const uint32_t C = 64 * W;                       // multiple of 64: 16-byte loads of four entries
+    const uint4* fh = reinterpret_cast<const uint4*>(d.first_hit + (size_t)inst * C);
     unsigned long long m = ~0ull;
-    for (uint32_t c = threadIdx.x; c < C; c += blockDim.x) {
-        const unsigned long long v = ((unsigned long long)fh[c] << 32) | c;
-        m = v < m ? v : m;
+    for (uint32_t q = threadIdx.x; q < C / 4; q += FIN_THREADS) {
+        const uint4 v = fh[q];
+        const uint32_t t[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const unsigned long long key = ((unsigned long long)t[k] << 32) | (4u * q + k);
+            m = key < m ? key : m;
+        }
     }
     for (int o = 16; o > 0; o >>= 1) {
         const unsigned long long v = __shfl_xor_sync(0xFFFFFFFFu, m, o);
@@ -192,7 +197,7 @@ __global__ void __launch_bounds__(256) k_finalize(DevPtrs d, uint32_t W, uint32_
     if ((threadIdx.x & 31) == 0) best[threadIdx.x >> 5] = m;
     __syncthreads();
     if (threadIdx.x == 0) {
-        for (uint32_t q = 1; q < blockDim.x / 32; ++q) m = best[q] < m ? best[q] : m;
+        for (uint32_t q = 1; q < FIN_THREADS / 32; ++q) m = best[q] < m ? best[q] : m;
         xs_tts_rec r = d.rec[inst];
         const bool skipped = r.solved && !(flags & XS_FLAG_NO_SKIP);
         if (!skipped) r.sweeps_done += n_sweeps;
@@ -863,9 +868,14 @@ static int launch_unsat_or(const xs_batch& b, cudaStream_t st)
 {
     const xs_params& p = b.p;
     XS_CU(cudaMemsetAsync(b.d.det, 0, (size_t)p.n_instances * p.n_words * 8, st));
-    dim3 grid((p.n_spins + DET_CHUNK - 1) / DET_CHUNK, p.n_instances);
     const uint32_t thr = std::min(256u, round_up(p.n_words, 32));
-    k_unsat_or<<<grid, thr, 0, st>>>(b.d, p.n_spins, p.n_words, b.d.det);
+    const uint32_t wblocks = std::min(64u, (p.n_words + thr - 1) / thr);
+    // clauses per CTA: 64, fewer when that leaves SMs without a CTA (small single instances)
+    const uint64_t ctas64 = (uint64_t)((p.n_spins + 63) / 64) * p.n_instances * wblocks;
+    uint32_t chunk = 64;
+    while (chunk > 4 && ctas64 * (64 / chunk) < 2ull * b.num_sms) chunk /= 2;
+    dim3 grid((p.n_spins + chunk - 1) / chunk, p.n_instances, wblocks);
+    k_unsat_or<<<grid, thr, 0, st>>>(b.d, p.n_spins, p.n_words, chunk, b.d.det);
     count_launch(1);
     return (int)cudaGetLastError();
 }
@@ -885,7 +895,7 @@ int launch_mark(const xs_batch& b, bool reset_first_hit, void* stream)
 
 int launch_finalize(const xs_batch& b, uint32_t n_sweeps, void* stream)
 {
-    k_finalize<<<b.p.n_instances, 256, 0, (cudaStream_t)stream>>>(b.d, b.p.n_words, n_sweeps, b.p.flags);
+    k_finalize<<<b.p.n_instances, FIN_THREADS, 0, (cudaStream_t)stream>>>(b.d, b.p.n_words, n_sweeps, b.p.flags);
     count_launch(1);
     return (int)cudaGetLastError();
 }

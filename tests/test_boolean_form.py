@@ -52,3 +52,55 @@ def test_boolean_update_equals_pm1_rule_on_all_inputs():
         assert lop3(L["LUT_NZ"], M, P, x) == int(k != 0), bits
         assert 2 * (M ^ x) + (P ^ x) == k, bits                    # the bit-sliced adder
         assert 6 - 4 * k in (6, 2, -2, -6)                         # Delta E of the flip (L67)
+
+
+def _src(name):
+    return open(os.path.join(ROOT, "paper_2102_09510_b200", "csrc", name)).read()
+
+
+def test_clause_word_forms_equal_pm1_rule_on_all_inputs():
+    """The clause-word kernels (xs_sweep_clause.cuh, xs_sweep_warp.cu) update from the three clause
+    bits c_r = x ^ a_r ^ b_r ^ j_r (1 <=> interaction r unsatisfied, L65-L67): k = c_0 + c_1 + c_2,
+    flip iff k >= 2 or (k = 1 and R) (L101), and a flip toggles the spin and its three clauses.
+    LUT constants and operand orders are read from the CUDA sources."""
+    L = _luts()
+    cl = _src("xs_sweep_clause.cuh")
+    m = re.search(r"constexpr int LUT_OR_ANDN = (0x[0-9A-Fa-f]+);", cl)
+    assert m
+    or_andn = int(m.group(1), 16)
+    assert re.search(r"M = lop3<LUT_MAJ>\(c0\[c\], c1\[c\], c2\[c\]\)", cl)
+    assert re.search(r"P = lop3<LUT_XOR3>\(c0\[c\], c1\[c\], c2\[c\]\)", cl)
+    assert re.search(r"f = lop3<LUT_OR_ANDN>\(M, P, nf\[c >> 1\]\)", cl)      # nf = NOT-flip mask (u >= thr)
+    assert re.search(r"c0\[c\] \^= f; c1\[c\] \^= f; c2\[c\] \^= f;\s*x\[r\]\[c\] \^= f;", cl)
+    m = re.search(r"PACK \? lop3<(0x[0-9A-Fa-f]+)>\(nb, rm\[r\], 0x80808080u\) : nb", cl)
+    assert m
+    merge = int(m.group(1), 16)
+    wp = _src("xs_sweep_warp.cu")
+    pat = r"wp_sts\(ca\[r\]\[%d\], lop3<LUT_SEL>\(R, lop3<(0x[0-9A-Fa-f]+)>\(c0, c1, c2\), lop3<(0x[0-9A-Fa-f]+)>\(c0, c1, c2\)\)\);"
+    two = [tuple(int(v, 16) for v in re.search(pat % k, wp).groups()) for k in range(3)]
+    m = re.search(r"x\[r\] \^= lop3<LUT_SEL>\(R, lop3<(0x[0-9A-Fa-f]+)>\(c0, c1, c2\), lop3<LUT_MAJ>\(c0, c1, c2\)\);", wp)
+    assert m
+    lut_or = int(m.group(1), 16)
+    for bits in itertools.product((0, 1), repeat=11):
+        a0, b0, a1, b1, a2, b2, j0, j1, j2, x, R = bits
+        s = lambda v: 1 - 2 * v                                    # noqa: E731
+        unsat = [int(s(j) * s(x) * s(a) * s(b) == -1) for (a, b, j) in ((a0, b0, j0), (a1, b1, j1), (a2, b2, j2))]
+        k = sum(unsat)
+        flip = int((k >= 2) or (k == 1 and R == 1))
+        c = [x ^ a0 ^ b0 ^ j0, x ^ a1 ^ b1 ^ j1, x ^ a2 ^ b2 ^ j2]
+        assert c == unsat, bits                                    # clause bit = "unsatisfied"
+        # clause-word kernel: threshold bytes hold NOT R
+        M, P = lop3(L["LUT_MAJ"], *c), lop3(L["LUT_XOR3"], *c)
+        assert lop3(or_andn, M, P, 1 - R) == flip, bits
+        # after the flip the clause bits must be those of the new spin value
+        x_new = x ^ flip
+        c_new = [x_new ^ a0 ^ b0 ^ j0, x_new ^ a1 ^ b1 ^ j1, x_new ^ a2 ^ b2 ^ j2]
+        assert [ci ^ flip for ci in c] == c_new, bits
+        # latency kernel: both candidates of every new clause bit, then the select by R
+        for r in range(3):
+            cand_r1, cand_r0 = lop3(two[r][0], *c), lop3(two[r][1], *c)
+            assert lop3(L["LUT_SEL"], R, cand_r1, cand_r0) == c_new[r], bits
+        assert lop3(L["LUT_SEL"], R, lop3(lut_or, *c), M) == flip, bits
+    # the merge of new threshold bits into the register that also carries the spin index
+    for a, b, cc in itertools.product((0, 1), repeat=3):
+        assert lop3(merge, a, b, cc) == (a if cc else b)
