@@ -5,7 +5,8 @@
 // sets of mutually non-adjacent spins, permutation array + set sizes, N x 6 adjacency.
 // Readings: configuration model on 3N stubs shuffled by sorting Philox keys,
 // whole-attempt rejection; gauge bits from Philox; ascending scan order for the greedy sets.
-// Written independently of oracle/ -- the two must agree byte for byte (tests/test_generator.py).
+// Written independently of oracle/ -- the two must agree byte for byte
+// (tests/test_abi_cpu.py::test_generator_matches_oracle_generator).
 #include <algorithm>
 #include <numeric>
 

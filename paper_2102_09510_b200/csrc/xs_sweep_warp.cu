@@ -34,6 +34,7 @@ constexpr uint32_t WP_PROD = 3;       // producer warps
 constexpr uint32_t WP_KB = 32;        // sweeps per noise chunk = detection batch
 constexpr uint32_t WP_IDLE = 0xFFFFFFFFu;
 constexpr uint32_t WP_SMEM_MAX = 227u * 1024u;
+constexpr int LUT_OR_AND = 0xF8;   // a | (b & c)
 
 struct WarpArgs {
     DevPtrs d;
@@ -178,13 +179,13 @@ __global__ void __launch_bounds__(32 * (4 + WP_PROD), 1) k_sweep_warp(WarpArgs A
             if (r < (int)A.n_pass) {
                 const uint32_t c0 = wp_lds(ca[r][0]), c1 = wp_lds(ca[r][1]), c2 = wp_lds(ca[r][2]);
                 const uint32_t R = wp_lds(nrow + ((uint32_t)r * WP_SLOTS + slot) * W * 4u);
-                // flip = R ? (k >= 1) : (k >= 2) = R ? (c0 | c1 | c2) : maj(c0, c1, c2) (a-7).  Two
-                // levels of logic instead of three on the way to the stores: both candidates of
-                // every new clause word first (c ^ maj, c ^ or), then the select by R.
-                wp_sts(ca[r][0], lop3<LUT_SEL>(R, lop3<0x0E>(c0, c1, c2), lop3<0x18>(c0, c1, c2)));
-                wp_sts(ca[r][1], lop3<LUT_SEL>(R, lop3<0x32>(c0, c1, c2), lop3<0x24>(c0, c1, c2)));
-                wp_sts(ca[r][2], lop3<LUT_SEL>(R, lop3<0x54>(c0, c1, c2), lop3<0x42>(c0, c1, c2)));
-                x[r] ^= lop3<LUT_SEL>(R, lop3<0xFE>(c0, c1, c2), lop3<LUT_MAJ>(c0, c1, c2));
+                const uint32_t M = lop3<LUT_MAJ>(c0, c1, c2);       // k >= 2
+                const uint32_t P = lop3<LUT_XOR3>(c0, c1, c2);      // k odd
+                const uint32_t f = lop3<LUT_OR_AND>(M, P, R);       // flip mask (a-7)
+                wp_sts(ca[r][0], c0 ^ f);
+                wp_sts(ca[r][1], c1 ^ f);
+                wp_sts(ca[r][2], c2 ^ f);
+                x[r] ^= f;
                 __syncwarp();                                        // a-8
             }
         }

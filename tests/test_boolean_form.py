@@ -76,11 +76,11 @@ def test_clause_word_forms_equal_pm1_rule_on_all_inputs():
     assert m
     merge = int(m.group(1), 16)
     wp = _src("xs_sweep_warp.cu")
-    pat = r"wp_sts\(ca\[r\]\[%d\], lop3<LUT_SEL>\(R, lop3<(0x[0-9A-Fa-f]+)>\(c0, c1, c2\), lop3<(0x[0-9A-Fa-f]+)>\(c0, c1, c2\)\)\);"
-    two = [tuple(int(v, 16) for v in re.search(pat % k, wp).groups()) for k in range(3)]
-    m = re.search(r"x\[r\] \^= lop3<LUT_SEL>\(R, lop3<(0x[0-9A-Fa-f]+)>\(c0, c1, c2\), lop3<LUT_MAJ>\(c0, c1, c2\)\);", wp)
+    m = re.search(r"constexpr int LUT_OR_AND = (0x[0-9A-Fa-f]+);", wp)
     assert m
-    lut_or = int(m.group(1), 16)
+    or_and = int(m.group(1), 16)
+    assert re.search(r"f = lop3<LUT_OR_AND>\(M, P, R\)", wp)                  # R = flip mask (u < thr)
+    assert re.search(r"wp_sts\(ca\[r\]\[0\], c0 \^ f\);\s*wp_sts\(ca\[r\]\[1\], c1 \^ f\);\s*wp_sts\(ca\[r\]\[2\], c2 \^ f\);\s*x\[r\] \^= f;", wp)
     for bits in itertools.product((0, 1), repeat=11):
         a0, b0, a1, b1, a2, b2, j0, j1, j2, x, R = bits
         s = lambda v: 1 - 2 * v                                    # noqa: E731
@@ -96,11 +96,8 @@ def test_clause_word_forms_equal_pm1_rule_on_all_inputs():
         x_new = x ^ flip
         c_new = [x_new ^ a0 ^ b0 ^ j0, x_new ^ a1 ^ b1 ^ j1, x_new ^ a2 ^ b2 ^ j2]
         assert [ci ^ flip for ci in c] == c_new, bits
-        # latency kernel: both candidates of every new clause bit, then the select by R
-        for r in range(3):
-            cand_r1, cand_r0 = lop3(two[r][0], *c), lop3(two[r][1], *c)
-            assert lop3(L["LUT_SEL"], R, cand_r1, cand_r0) == c_new[r], bits
-        assert lop3(L["LUT_SEL"], R, lop3(lut_or, *c), M) == flip, bits
+        # latency kernel: the same with the mask R itself
+        assert lop3(or_and, M, P, R) == flip, bits
     # the merge of new threshold bits into the register that also carries the spin index
     for a, b, cc in itertools.product((0, 1), repeat=3):
         assert lop3(merge, a, b, cc) == (a if cc else b)
