@@ -53,7 +53,7 @@ WORKLOADS = {
     "config2_metropolis": dict(N=256, W=1024, I=1, sweeps=1_000, graph_seed=2, run_seed=2, balanced=True, set_cap=64,
                                metropolis=True,
                                desc="configs[1] with the Metropolis table w0 = w1^3, w2 = w3 = 1 (L69) at w1 = 0.055: N=256, "
-                                    "2^16 clones, 1000 sweeps per step, first hits looked for after every sweep"),
+                                    "2^16 clones, 1000 sweeps per step, first hits looked for after every sweep (clause-word kernel, W0 form)"),
     "config1": dict(N=64, W=1, I=1, sweeps=10_000, graph_seed=1, run_seed=1,
                     desc="configs[0] shape: N=64, 1 instance (graph seed 1), 64 clones, 10^4 sweeps per step, no early stop "
                          "(latency: one warp of work)"),

@@ -157,8 +157,9 @@ int xs_run_sweeps(xs_batch* b, uint64_t n_sweeps, void* cuda_stream);
  * w0 = w1^3, w2 = w3 = 1 satisfies detailed balance (Metropolis at T = -2 / ln w1).
  * thr4[k] in [0, 2^32] (host array): the spin flips iff the word's 32-bit number u < thr4[k];
  * the same u serves every k (L87).  Takes effect from the next xs_run_sweeps; the default after
- * xs_create_instance* is (0, w1_threshold, 2^32, 2^32).  Tables that are not of the quasi-greedy
- * form run on the generic / streaming kernels; with thr4[0] > 0 a ground state can be left
+ * xs_create_instance* is (0, w1_threshold, 2^32, 2^32).  The quasi-greedy form and, on balanced
+ * sets that fill the CTA, the family (w0, w1, 1, 1) with 0 < w0 <= w1 (Metropolis) run on the
+ * clause-word kernel; other tables on the generic / streaming kernels; with thr4[0] > 0 a ground state can be left
  * again, so first hits are looked for after every sweep.  The launch geometry is chosen anew
  * (a table can move the batch to another kernel); tables a kernel needs are uploaded on
  * cuda_stream, which is synchronised if an upload happens. */
@@ -206,8 +207,11 @@ int xs_generate_graph(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uin
  * (L277: the spins of a set may be updated in any order, or concurrently).  Outputs:
  *   task   [*n_rounds * n_slots][4] (room for 2 N entries): entry e = round * n_slots + slot ->
  *                  byte offsets of the spin's three clause rows (128 t + 64 half_t, in the order
- *                  the kernel accesses them) and the spin index; spin = 0xFFFFFFFF: the slot is idle
- *                  in that round and its offsets point into scratch line N + slot / 2;
+ *                  the kernel accesses them) and, in bits 0-15, the spin index; bit 16 + k is set iff
+ *                  this round is the last of the sweep that touches the entry's clause k (the kernels
+ *                  for flip tables with w0 > 0 look for ground states there); the whole word =
+ *                  0xFFFFFFFF: the slot is idle in that round and its offsets point into scratch line
+ *                  N + slot / 2;
  *   place  [N]   : byte offset of clause t's row;
  *   *barrier_mask: bit r set <=> round r is the last round of its set (barrier after it).
  * Guarantees: every spin of a set appears exactly once among the entries of the set's rounds, and

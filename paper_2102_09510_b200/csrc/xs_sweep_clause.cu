@@ -25,7 +25,7 @@ constexpr uint32_t CL_SMEM_MAX = 227u * 1024u;
 inline uint32_t clause_off_misc(uint32_t N, uint32_t n_slots) { return (N + n_slots / 2u) * 128u; }
 inline uint32_t clause_smem(uint32_t N, uint32_t n_slots)
 {
-    return clause_off_misc(N, n_slots) + (4u * CL_T + 4u) * 4u + 128u;
+    return clause_off_misc(N, n_slots) + (6u * CL_T + 4u) * 4u + 128u;
 }
 
 struct Rng {
@@ -177,6 +177,24 @@ bool clause_placement(const HostGraph& g, uint32_t n_slots, uint32_t n_rounds, C
             crec[(size_t)r * n_slots + 2 * m + 1] = CRec{scratch | 64u, scratch | 64u, scratch | 64u, CL_IDLE};
             any_idle = true;
         }
+    // bits 16-18 of an entry's spin field: this round is the LAST touch of its clause 0 / 1 / 2 in a
+    // sweep (the kernels for tables with w0 > 0 OR the clause words there: all clear <=> E = -N)
+    {
+        std::vector<uint32_t> round_of(N, 0), last_round(N, 0);
+        for (uint32_t e = 0; e < round0 * n_slots; ++e)
+            if (crec[e].spin != CL_IDLE) round_of[crec[e].spin] = e / n_slots;
+        for (uint32_t t = 0; t < N; ++t)
+            last_round[t] = std::max({round_of[g.tri[3ull * t]], round_of[g.tri[3ull * t + 1]],
+                                      round_of[g.tri[3ull * t + 2]]});
+        for (uint32_t e = 0; e < round0 * n_slots; ++e) {
+            CRec& c = crec[e];
+            if (c.spin == CL_IDLE) continue;
+            const uint32_t r = e / n_slots;
+            const uint32_t off[3] = {c.off0, c.off1, c.off2};
+            for (int k = 0; k < 3; ++k)
+                if (last_round[off[k] >> 7] == r) c.spin |= 1u << (16 + k);
+        }
+    }
     if (bar_mask) *bar_mask = bm;
     if (mode) *mode = any_idle ? 0u : all_one ? 1u : all_two ? 2u : 0u;
     return true;
@@ -189,7 +207,11 @@ int clause_prepare(xs_batch& b, void* stream)
     TileGeom& g = b.geom;
     const xs_geometry& rq = b.req;
     if (rq.variant != XS_GEOM_AUTO && rq.variant != 2u) return 0;   // another kernel was asked for
-    if (g.regime != 0 || b.ft.general || b.ft.per_clone || (b.p.flags & XS_FLAG_STREAMING)) return 0;
+    if (g.regime != 0 || b.ft.per_clone || (b.p.flags & XS_FLAG_STREAMING)) return 0;
+    // flip tables: the quasi-greedy form (0, w1, 1, 1) and, on full lists (MODE 1), the family
+    // (w0, w1, 1, 1) with 0 < w0 <= w1 (L69: Metropolis w0 = w1^3); anything else: generic kernel
+    const bool family = b.ft.general && b.ft.always == 0xCu && b.ft.lo[0] > 0u && b.ft.lo[0] <= b.ft.lo[1];
+    if (b.ft.general && !family) return 0;
     if (rq.tile_words && rq.tile_words != CL_T) return 0;
     const uint32_t N = b.p.n_spins, I = b.p.n_instances, W = b.p.n_words;
     if (W % CL_T || N < 64u || N >= (1u << 14)) return 0;
@@ -243,6 +265,7 @@ int clause_prepare(xs_batch& b, void* stream)
         b.clause_rounds = rounds;
         b.clause_mode = mode == 3 ? 0u : mode;
     }
+    if (family && b.clause_mode != 1u) return 0;      // w0 > 0 needs the full lists
     if (b.clause_thr != (uint64_t)b.p.w1_threshold) {
         // compare constants of the noise (xs_sweep_clause.cuh): 2^32 - thr, and the forced carry for thr = 0
         const uint32_t h[2] = {0u - b.p.w1_threshold, b.p.w1_threshold == 0u ? 1u : 0u};
@@ -275,11 +298,13 @@ int launch_sweep_clause(const xs_batch& b, uint32_t n_sweeps, void* stream)
     A.n_slots = g.threads / CL_LPS;
     A.ent = crec_entries(b.p);
     A.off_misc = clause_off_misc(b.p.n_spins, A.n_slots);
-    A.thr = b.p.w1_threshold;
+    A.thr = b.ft.general ? b.ft.lo[1] : b.p.w1_threshold;
+    A.thr0 = b.ft.general ? b.ft.lo[0] : 0u;
     A.one = 1u;
     A.zero = 0u;
     ClauseLaunch L;
     L.threads = g.threads; L.smem = g.smem; L.mode = b.clause_mode;
+    L.w0 = b.ft.general != 0u;
     L.dense = g.ctas > b.num_sms;
     L.st = (cudaStream_t)stream;
     const uint32_t tiles = b.p.n_words / CL_T;

@@ -63,6 +63,7 @@ struct ClauseArgs {
     uint32_t inst0;          // first instance of this launch
     uint32_t off_misc;       // byte offset of det32 / known32 / flag in dynamic shared memory
     uint32_t thr;            // noise threshold: a k = 1 spin flips iff u < thr
+    uint32_t thr0;           // W0 kernels: a k = 0 spin flips iff u < thr0 (thr0 <= thr)
     uint32_t one;            // the multiplier 1, as data, so that the compare stays a multiply-add
     uint32_t zero;           // the multiplier 0, as data: ties the last store of a round to its Philox call
     uint64_t seed[CL_MAXI];  // run seeds of instances inst0 .. (constant bank -> uniform registers)
@@ -103,7 +104,12 @@ constexpr int LUT_OR_ANDN = 0xF4;   // a | (b & ~c)
 //         round) and the barriers follow the per-instance mask cbar (bit r: barrier after round r);
 // MODE 1: every slot has a spin in every round, barrier after every round (R sets of n_slots);
 // MODE 2: every slot busy, barrier after every second round (R / 2 sets of 2 n_slots spins).
-template <int R, int MAXTHREADS, int MINB, int MODE>
+// W0: flip table (w0, w1, 1, 1) with 0 < w0 <= w1 (the Metropolis table w0 = w1^3;
+//     SURVEY.md 8(f) NEXT-1), MODE 1 only.  A k = 0 spin flips iff the word's number u < thr0, so a second
+//     threshold bit per word is kept (flip = M | (P & u<thr) | u<thr0), and a ground state can be
+//     left again: the first hit is looked for after EVERY sweep, without extra loads, by OR-ing
+//     every clause word at its LAST touch of the sweep (a static 3-bit mask per task, from the host).
+template <int R, int MAXTHREADS, int MINB, int MODE, bool W0 = false>
 __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_constant__ ClauseArgs A)
 {
     // One CTA per SM with few warps (fewer tiles than SMs, e.g. BASELINE.json configs[1]): the
@@ -122,7 +128,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
 
     const uint32_t base = (uint32_t)__cvta_generic_to_shared(smem);
     uint32_t* det32 = reinterpret_cast<uint32_t*>(smem + A.off_misc);
-    uint32_t* known32 = det32 + 2 * CL_T;
+    uint32_t* known32 = det32 + 4 * CL_T;         // det32: two buffers of 2 T words (W0: by sweep parity)
     uint32_t* flag = known32 + 2 * CL_T;
 
     const uint32_t n_slots = A.n_slots;
@@ -150,6 +156,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     auto spin_of = [&](int r) -> uint32_t {
         return PACK ? ((rm[r] & 0x7Fu) | ((rm[r] >> 1) & 0x3F80u)) : spin[PACK ? 0 : r];
     };
+    uint32_t rm0[W0 ? R : 1];         // W0: the same bytes for the k = 0 threshold
+    uint32_t last = 0;                // W0: bit 3 r + k <=> round r is the last touch of its clause k in a sweep
     uint32_t act = 0, wact = 0, bar = 0;
     {
         const uint4* cr = reinterpret_cast<const uint4*>(A.d.crec + (size_t)inst * A.ent);
@@ -163,7 +171,11 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
                 rm[r] = (v.w & 0x7Fu) | ((v.w & 0x3F80u) << 1);
             } else {
                 rm[r] = 0;
-                spin[PACK ? 0 : r] = v.w;
+                spin[PACK ? 0 : r] = v.w & 0xFFFFu;      // bits 16-18: last-touch mask
+            }
+            if (W0) {
+                rm0[r] = 0;
+                last |= ((v.w >> 16) & 7u) << (3 * r);
             }
             if (MODE == 0) {
                 const bool a = v.w != CL_IDLE;
@@ -204,6 +216,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
                     make_uint4(x[r][0], x[r][1], x[r][2], x[r][3]);
     };
     load_state();
+    for (uint32_t e = threadIdx.x; e < 4 * CL_T; e += blockDim.x) det32[e] = 0;
     for (uint32_t e = threadIdx.x; e < 64 * CL_T; e += blockDim.x) {
         const bool kn = fhg[e] != XS_NO_HIT;
         const uint32_t m = __ballot_sync(0xFFFFFFFFu, kn);
@@ -232,7 +245,16 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
         uint32_t o[4];
         philox4x32_10(spin_of(r), grp, 2u * k - (uint32_t)(r & 1) + jl, TAG_SWEEP, k0, k1, o);
         uint32_t v = 0;
-        if (SPARSE) {
+        if (W0) {
+            const uint32_t thr = A.thr, thr0 = A.thr0;
+            v = (o[0] >= thr ? 0xFFu : 0u) | (o[1] >= thr ? 0xFF00u : 0u) |
+                (o[2] >= thr ? 0xFF0000u : 0u) | (o[3] >= thr ? 0xFF000000u : 0u);
+            const uint32_t v0 = (o[0] >= thr0 ? 0xFFu : 0u) | (o[1] >= thr0 ? 0xFF00u : 0u) |
+                                (o[2] >= thr0 ? 0xFF0000u : 0u) | (o[3] >= thr0 ? 0xFF000000u : 0u);
+            const uint32_t z0 = __shfl_sync(0xFFFFFFFFu, v0, lane_base);
+            const uint32_t z1 = __shfl_sync(0xFFFFFFFFu, v0, lane_base + 1);
+            rm0[W0 ? r : 0] = cl_prmt(z0, z1, sub_sel);
+        } else if (SPARSE) {
             // plain compares: the shortest dependent chain (set-predicate, select, OR)
             const uint32_t thr = A.thr;
             v = (o[0] >= thr ? 0xFFu : 0u) | (o[1] >= thr ? 0xFF00u : 0u) |
@@ -265,6 +287,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     // in the latency shadow of the round's loads. ------------------------------------------------
     auto sweep = [&](auto hc, uint32_t t) {
         constexpr uint32_t h = decltype(hc)::value;
+        uint32_t lacc[CL_H] = {0u, 0u, 0u, 0u};      // W0: OR of the clause words at their last touch
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             if (MODE != 0 || ((wact >> r) & 1u)) {
@@ -275,6 +298,11 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
                 uint32_t nf[2];
                 nf[0] = cl_prmt(rm[r], 0u, sel0);
                 nf[1] = cl_prmt(rm[r], 0u, sel0 + 0x1111u);
+                uint32_t n0[2] = {0u, 0u};
+                if (W0) {
+                    n0[0] = cl_prmt(rm0[W0 ? r : 0], 0u, sel0);
+                    n0[1] = cl_prmt(rm0[W0 ? r : 0], 0u, sel0 + 0x1111u);
+                }
                 // The address of the round's last store is made to depend (times zero) on the call's
                 // result: the instruction scheduler then treats the Philox chain as the critical path
                 // of the round and issues it first, interleaved with the update, in the shadow of
@@ -289,14 +317,52 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
                 for (int c = 0; c < CL_H; ++c) {
                     const uint32_t M = lop3<LUT_MAJ>(c0[c], c1[c], c2[c]);     // k >= 2
                     const uint32_t P = lop3<LUT_XOR3>(c0[c], c1[c], c2[c]);    // k odd
-                    const uint32_t f = lop3<LUT_OR_ANDN>(M, P, nf[c >> 1]);    // flip mask (a-7)
+                    uint32_t f = lop3<LUT_OR_ANDN>(M, P, nf[c >> 1]);          // flip mask (a-7)
+                    if (W0) f = lop3<0xF3>(f, n0[c >> 1], 0u);                 // | (u < thr0): the k = 0 move
                     c0[c] ^= f; c1[c] ^= f; c2[c] ^= f;
                     x[r][c] ^= f;
                 }
+                if (W0) {
+                    const uint32_t l0 = 0u - ((last >> (3 * r)) & 1u), l1 = 0u - ((last >> (3 * r + 1)) & 1u),
+                                   l2 = 0u - ((last >> (3 * r + 2)) & 1u);
+#pragma unroll
+                    for (int c = 0; c < CL_H; ++c) {
+                        lacc[c] = lop3<0xEA>(c0[c], l0, lacc[c]);              // (a & b) | c
+                        lacc[c] = lop3<0xEA>(c1[c], l1, lacc[c]);
+                        lacc[c] = lop3<0xEA>(c2[c], l2, lacc[c]);
+                    }
+                }
                 cl_sts4(ca[r][0], c0); cl_sts4(ca[r][1], c1); cl_sts4(a2, c2);
+            }
+            if (W0 && r == R - 1) {
+                // every clause word has had its last touch: clones with a set bit are not in a ground state
+                uint32_t* det = det32 + (t & 1u) * 2u * CL_T;
+#pragma unroll
+                for (int c = 0; c < CL_H; ++c) {
+                    lacc[c] |= __shfl_xor_sync(0xFFFFFFFFu, lacc[c], 4);
+                    lacc[c] |= __shfl_xor_sync(0xFFFFFFFFu, lacc[c], 8);
+                    lacc[c] |= __shfl_xor_sync(0xFFFFFFFFu, lacc[c], 16);
+                    if ((threadIdx.x & 31u) < CL_LPS && lacc[c]) atomicOr(&det[CL_H * j + c], lacc[c]);
+                }
             }
             if (MODE == 1 || (MODE == 2 && (r & 1)) || (MODE == 0 && ((bar >> r) & 1u)))
                 __syncthreads();                                              // a-8
+        }
+    };
+
+    // W0: after the last barrier of sweep t, record the clones whose clause words are all clear and
+    // clear the buffer for sweep t + 2
+    auto w0_commit = [&](uint32_t t) {
+        uint32_t* det = det32 + (t & 1u) * 2u * CL_T;
+        for (uint32_t e = threadIdx.x; e < 2 * CL_T; e += blockDim.x) {
+            uint32_t newly = ~det[e] & ~known32[e];
+            det[e] = 0;
+            known32[e] |= newly;
+            while (newly) {
+                const int bit = __ffs(newly) - 1;
+                newly &= newly - 1;
+                fhg[32 * e + bit] = t;
+            }
         }
     };
 
@@ -324,6 +390,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     // sweeps t0+1 .. t0+n; exact: record first hits after every sweep (L293)
     auto run_range = [&](uint32_t t0, uint32_t n, bool exact) {
         auto post = [&](uint32_t t) {
+            if (W0) { w0_commit(t); return; }
             if (!exact) return;
             detect();
             for (uint32_t e = threadIdx.x; e < 2 * CL_T; e += blockDim.x) {
@@ -362,6 +429,12 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     while (remaining) {
         const uint32_t nb = min(A.batch, remaining);
         run_range(t, nb, false);
+        if (W0) {                  // first hits are already exact; no detection pass, no replay
+            store_state();
+            t += nb;
+            remaining -= nb;
+            continue;
+        }
         detect();
         for (uint32_t e = threadIdx.x; e < 2 * CL_T; e += blockDim.x)
             if (~det32[e] & ~known32[e]) *flag = 1;
@@ -382,23 +455,25 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
 // ---- launch of one R family; each family is instantiated in its own translation unit ---------
 struct ClauseLaunch {
     uint32_t threads, ctas, smem, mode;
+    bool w0;             // flip table with w0 > 0 (MODE 1 only)
     bool dense;          // more CTAs than SMs: prefer the register-capped variants
     cudaStream_t st;
 };
 
-template <int R, int MT, int MINB, int MODE>
+template <int R, int MT, int MINB, int MODE, bool W0 = false>
 cudaError_t launch_clause_k(const ClauseArgs& A, const ClauseLaunch& L)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_clause<R, MT, MINB, MODE>,
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_clause<R, MT, MINB, MODE, W0>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem);
     if (e != cudaSuccess) return e;
-    k_sweep_clause<R, MT, MINB, MODE><<<L.ctas, L.threads, L.smem, L.st>>>(A);
+    k_sweep_clause<R, MT, MINB, MODE, W0><<<L.ctas, L.threads, L.smem, L.st>>>(A);
     return cudaGetLastError();
 }
 
 template <int R, int MT, int MINB>
 cudaError_t launch_clause_m(const ClauseArgs& A, const ClauseLaunch& L)
 {
+    if (L.mode == 1 && L.w0) return launch_clause_k<R, MT, MINB, 1, true>(A, L);
     if (L.mode == 1) return launch_clause_k<R, MT, MINB, 1>(A, L);
     if (L.mode == 2 && R % 2 == 0) return launch_clause_k<R, MT, MINB, (R % 2 == 0 ? 2 : 0)>(A, L);
     return launch_clause_k<R, MT, MINB, 0>(A, L);

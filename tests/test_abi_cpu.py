@@ -99,6 +99,9 @@ def test_clause_placement_is_conflict_free_and_complete(N, seed, n_slots, balanc
         for v in (i, j, k):
             clauses_of[v].append(c)
     IDLE = 0xFFFFFFFF
+    raw = task.copy()
+    last_bits = np.where(task[:, 3] != IDLE, (task[:, 3] >> 16) & 7, 0)
+    task[:, 3] = np.where(task[:, 3] != IDLE, task[:, 3] & 0xFFFF, IDLE)     # bits 16-18: last-touch mask
     r0, p0, want_bar = 0, 0, 0
     for sz in ss.tolist():
         nr = -(-sz // n_slots)
@@ -117,11 +120,20 @@ def test_clause_placement_is_conflict_free_and_complete(N, seed, n_slots, balanc
             assert ((e[:3] >> 7) == N + (e_i % n_slots) // 2).all()       # scratch line of the slot pair
     half = (task[:, :3] >> 6) & 1
     assert ((half[0::2] ^ half[1::2]) == 1).all()
+    # last-touch mask: bit k of an entry <=> no later round of the sweep touches its clause k
+    round_of = {int(e[3]): i // n_slots for i, e in enumerate(task) if e[3] != IDLE}
+    for i, e in enumerate(task):
+        if e[3] == IDLE:
+            continue
+        for k in range(3):
+            members = tri[int(e[k]) >> 7].tolist()
+            is_last = max(round_of[m] for m in members) == i // n_slots
+            assert ((int(last_bits[i]) >> k) & 1) == int(is_last)
     if balanced and cap == 0 and N % (n_slots * 4) == 0 and len(ss) * n_slots == N:
         assert (task[:, 3] != IDLE).all()                                 # full sets: no idle slot
     # deterministic
     task2, place2, bar2 = xs.xs_clause_placement(N, seed, n_slots, fl, cap)
-    assert np.array_equal(task, task2) and np.array_equal(place, place2) and bar == bar2
+    assert np.array_equal(raw, task2) and np.array_equal(place, place2) and bar == bar2
 
 
 def test_clause_placement_rejects_orders_that_do_not_fit():

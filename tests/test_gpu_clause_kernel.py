@@ -88,7 +88,7 @@ def test_clause_kernel_multi_instance_stop_rule_and_flip_table_switch():
     seeds = [900 + i for i in range(I)]
     b = xs.Batch(N, W, seeds, seeds, flags=xs.XS_FLAG_GAUGE | xs.XS_FLAG_BALANCED)
     assert b.layout().variant == 2 and b.layout().ctas == I
-    b.set_flip_table([1 << 20, 236223201, 1 << 32, 1 << 32])     # general table: generic kernel
+    b.set_flip_table([0, 236223201, 1 << 31, 1 << 32])           # w2 < 1: general table, generic kernel
     assert b.layout().variant == 0
     b.set_flip_table([0, 236223201, 1 << 32, 1 << 32])           # back to quasi-greedy
     assert b.layout().variant == 2

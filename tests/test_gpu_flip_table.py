@@ -99,3 +99,52 @@ def test_back_to_quasi_greedy_table_uses_fast_kernel():
     with pytest.raises(xs.XsError):
         b.set_flip_table([0, 1, 2, TWO32 + 1])
     b.close()
+
+
+@pytest.mark.parametrize("N,W,I,T", [(128, 8, 1, 0.69), (128, 16, 3, 1.2), (192, 8, 2, 0.69), (256, 8, 1, 2.0), (512, 8, 1, 0.9)])
+def test_w0_family_on_the_clause_word_kernel(N, W, I, T):
+    """SURVEY.md 8(f) NEXT-1 on the fast kernel: tables (w0, w1, 1, 1) with 0 < w0 <= w1 (L69: Metropolis,
+    w0 = w1^3) run on the clause-word kernel when the balanced sets fill the CTA; ground states are not
+    absorbing, so the kernel looks for first hits after every sweep (OR of the clause words at their last
+    touch).  Clones start a few flips away from the planted state so that they enter and leave E = -N."""
+    import paper_2102_09510_b200 as xs
+    t4 = metropolis(T)
+    assert 0 < t4[0] <= t4[1] < TWO32 and t4[2] == t4[3] == TWO32
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_BALANCED
+    gs, rs = [N + 40 + i for i in range(I)], [3 * N + i for i in range(I)]
+    b = xs.Batch(N, W, gs, rs, flags=fl, geometry=dict(batch_sweeps=16))
+    b.set_flip_table(t4)
+    lay = b.layout()
+    assert (lay.regime, lay.variant, lay.tile_words) == (0, 2, 8), (lay.regime, lay.variant, lay.tile_words)
+    os_ = [OracleRun(N, W, g, r, no_skip=True, thr4=t4, balanced=True) for g, r in zip(gs, rs)]
+    rng = np.random.default_rng(11)
+    x = np.zeros((I, N, W), np.uint64)
+    for i, o in enumerate(os_):
+        taubit = o.inst.taubit.astype(np.uint64)
+        x[i] = (taubit * np.uint64(0xFFFFFFFFFFFFFFFF))[:, None]
+        for k in range(64):
+            x[i] ^= (rng.random((N, W)) < 0.02).astype(np.uint64) << np.uint64(k)
+        o.s = o.inst.unpack(x[i])
+        o.first_hit = o.inst.mark_initial(o.s)
+    b.set_spins(torch.from_numpy(x.view(np.int64)).cuda())
+    for n in (1, 2, 21, 40):
+        b.run_sweeps(n)
+        for o in os_:
+            o.run_sweeps(n)
+    xg, fh, e = b.spins_numpy(), b.first_hit_numpy(), b.energy().cpu().numpy()
+    for i, o in enumerate(os_):
+        assert np.array_equal(xg[i], o.x()), f"spins inst {i}"
+        assert np.array_equal(fh[i], o.first_hit), f"first hits inst {i}"
+        assert np.array_equal(e[i], o.energy()), f"energies inst {i}"
+    if T <= 0.9 and N <= 192:
+        hit = os_[0].first_hit != NO_HIT
+        assert hit.sum() > 10                       # the case really sees first hits ...
+    # back to the quasi-greedy table on the same batch: the plain kernel, still bit-exact
+    b.set_flip_table([0, 236223201, TWO32, TWO32])
+    assert b.layout().variant == 2
+    b.run_sweeps(9)
+    for i, o in enumerate(os_):
+        o.thr4 = None
+        o.run_sweeps(9)
+        assert np.array_equal(b.spins_numpy()[i], o.x()) and np.array_equal(b.first_hit_numpy()[i], o.first_hit)
+    b.close()
