@@ -202,7 +202,7 @@ int xs_generate_graph(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uin
  * instance xs_generate_graph builds from the same arguments.  The kernel keeps one
  * 64-byte row per interaction t, c_t = x_i ^ x_j ^ x_k ^ J_t (a spin's update
  * needs only the number of unsatisfied interactions it enters), in the lower or upper half of
- * 128-byte line t.  A sweep is *n_rounds rounds (>= 4, <= 8); a round puts one spin on each of the
+ * 128-byte line t.  A sweep is *n_rounds rounds (>= 4, <= 16); a round puts one spin on each of the
  * CTA's n_slots slots; an independent set of sz spins takes ceil(sz / n_slots) consecutive rounds
  * (L277: the spins of a set may be updated in any order, or concurrently).  Outputs:
  *   task   [*n_rounds * n_slots][4] (room for 2 N entries): entry e = round * n_slots + slot ->
@@ -216,7 +216,7 @@ int xs_generate_graph(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uin
  *   *barrier_mask: bit r set <=> round r is the last round of its set (barrier after it).
  * Guarantees: every spin of a set appears exactly once among the entries of the set's rounds, and
  * slots (2m, 2m+1), which share a shared-memory phase, touch opposite halves in each of their
- * three accesses.  XS_EINVAL if the order needs more than 8 rounds or more than 2 N entries on
+ * three accesses.  XS_EINVAL if the order needs more than 16 rounds or more than 2 N entries on
  * n_slots slots (n_slots even), or no placement was found.  Any output pointer may be NULL. */
 int xs_clause_placement(uint32_t n_spins, uint64_t graph_seed, uint32_t flags, uint32_t set_cap,
                         uint32_t n_slots, uint32_t* task, uint32_t* place, uint32_t* n_rounds,

@@ -16,10 +16,19 @@ extern template cudaError_t launch_clause_unit<5>(const ClauseArgs&, const Claus
 extern template cudaError_t launch_clause_unit<6>(const ClauseArgs&, const ClauseLaunch&);
 extern template cudaError_t launch_clause_unit<7>(const ClauseArgs&, const ClauseLaunch&);
 extern template cudaError_t launch_clause_unit<8>(const ClauseArgs&, const ClauseLaunch&);
+extern template cudaError_t launch_clause_unit_long<9>(const ClauseArgs&, const ClauseLaunch&);
+extern template cudaError_t launch_clause_unit_long<10>(const ClauseArgs&, const ClauseLaunch&);
+extern template cudaError_t launch_clause_unit_long<11>(const ClauseArgs&, const ClauseLaunch&);
+extern template cudaError_t launch_clause_unit_long<12>(const ClauseArgs&, const ClauseLaunch&);
+extern template cudaError_t launch_clause_unit_long<13>(const ClauseArgs&, const ClauseLaunch&);
+extern template cudaError_t launch_clause_unit_long<14>(const ClauseArgs&, const ClauseLaunch&);
+extern template cudaError_t launch_clause_unit_long<15>(const ClauseArgs&, const ClauseLaunch&);
+extern template cudaError_t launch_clause_unit_long<16>(const ClauseArgs&, const ClauseLaunch&);
 
 namespace {
 
-constexpr uint32_t CL_RMIN = 4, CL_RMAX = 8;      // rounds per sweep the kernel is instantiated for
+constexpr uint32_t CL_RMIN = 4, CL_RMAX = 16;     // rounds per sweep the kernel is instantiated for
+constexpr uint32_t CL_RCAP = 8;                   // ... under the 128-register cap of the dense launch classes
 constexpr uint32_t CL_SMEM_MAX = 227u * 1024u;
 
 inline uint32_t clause_off_misc(uint32_t N, uint32_t n_slots) { return (N + n_slots / 2u) * 128u; }
@@ -225,6 +234,7 @@ int clause_prepare(xs_batch& b, void* stream)
         for (const HostGraph& hg : b.graphs) r = std::max(r, clause_rounds(hg, ns));
         r = std::max(r, CL_RMIN);
         if (r > CL_RMAX || (uint64_t)r * ns > 2ull * N) continue;
+        if (r > CL_RCAP && thr > 256u) continue;           // long lists: CTAs of at most 256 threads
         if (r < rounds) { rounds = r; threads = thr; }
     }
     if (!threads) return 0;
@@ -265,7 +275,7 @@ int clause_prepare(xs_batch& b, void* stream)
         b.clause_rounds = rounds;
         b.clause_mode = mode == 3 ? 0u : mode;
     }
-    if (family && b.clause_mode != 1u) return 0;      // w0 > 0 needs the full lists
+    if (family && (b.clause_mode != 1u || rounds > CL_RCAP)) return 0;      // w0 > 0 needs the full lists
     if (b.clause_thr != (uint64_t)b.p.w1_threshold) {
         // compare constants of the noise (xs_sweep_clause.cuh): 2^32 - thr, and the forced carry for thr = 0
         const uint32_t h[2] = {0u - b.p.w1_threshold, b.p.w1_threshold == 0u ? 1u : 0u};
@@ -319,7 +329,15 @@ int launch_sweep_clause(const xs_batch& b, uint32_t n_sweeps, void* stream)
             case 5: e = launch_clause_unit<5>(A, L); break;
             case 6: e = launch_clause_unit<6>(A, L); break;
             case 7: e = launch_clause_unit<7>(A, L); break;
-            default: e = launch_clause_unit<8>(A, L); break;
+            case 8: e = launch_clause_unit<8>(A, L); break;
+            case 9: e = launch_clause_unit_long<9>(A, L); break;
+            case 10: e = launch_clause_unit_long<10>(A, L); break;
+            case 11: e = launch_clause_unit_long<11>(A, L); break;
+            case 12: e = launch_clause_unit_long<12>(A, L); break;
+            case 13: e = launch_clause_unit_long<13>(A, L); break;
+            case 14: e = launch_clause_unit_long<14>(A, L); break;
+            case 15: e = launch_clause_unit_long<15>(A, L); break;
+            default: e = launch_clause_unit_long<16>(A, L); break;
         }
         if (e != cudaSuccess) return (int)e;
         count_launch(1);

@@ -487,4 +487,13 @@ cudaError_t launch_clause_unit(const ClauseArgs& A, const ClauseLaunch& L)
     return launch_clause_m<R, 512, 1>(A, L);
 }
 
+// 9 .. 16 rounds per sweep (orders with many small sets, e.g. the paper's cap-32 sets, L279): the
+// general form only, without a register cap (one CTA of at most 256 threads per launch bound).
+template <int R>
+cudaError_t launch_clause_unit_long(const ClauseArgs& A, const ClauseLaunch& L)
+{
+    if (L.threads == 128) return launch_clause_k<R, 128, 1, 0>(A, L);
+    return launch_clause_k<R, 256, 1, 0>(A, L);
+}
+
 }  // namespace xs

@@ -80,7 +80,8 @@ def test_balanced_sets_match_oracle(N, seed, cap):
     (1024, 1024000, 128, True, 0),     # 4 sets of 256 on 128 slots: 8 rounds, barrier after every second
     (160, 3, 32, True, 0), (224, 4, 32, True, 0), (320, 5, 64, True, 0),     # 5 / 7 / 5 sets
     (256, 2, 64, False, 0), (512, 100, 128, False, 0), (128, 9, 32, False, 0),  # greedy, ragged sets
-    (100, 6, 32, True, 25), (200, 11, 64, False, 0)])
+    (100, 6, 32, True, 25), (200, 11, 64, False, 0),
+    (256, 2, 32, False, 32), (192, 5, 32, False, 32)])    # the paper's cap-32 sets (L279): 10+ rounds
 def test_clause_placement_is_conflict_free_and_complete(N, seed, n_slots, balanced, cap):
     """Placement tables of the clause-word kernel (include/xs.h), checked straight
     from the triplets: the entries of a set's rounds are exactly the set's spins (L277: any order
@@ -91,7 +92,7 @@ def test_clause_placement_is_conflict_free_and_complete(N, seed, n_slots, balanc
     tri, jbit, order, ss, att = xs.xs_generate_graph(N, seed, fl, cap)
     task, place, bar = xs.xs_clause_placement(N, seed, n_slots, fl, cap)
     n_rounds = len(task) // n_slots
-    assert 4 <= n_rounds <= 8 and n_rounds * n_slots <= 2 * N
+    assert 4 <= n_rounds <= 16 and n_rounds * n_slots <= 2 * N
     t = np.arange(N, dtype=np.uint32)
     assert np.array_equal(place & ~np.uint32(64), t << 7)                 # own line, lower or upper half
     clauses_of = [[] for _ in range(N)]
@@ -137,8 +138,8 @@ def test_clause_placement_is_conflict_free_and_complete(N, seed, n_slots, balanc
 
 
 def test_clause_placement_rejects_orders_that_do_not_fit():
-    with pytest.raises(xs.XsError):                     # sets of 64 on 16 slots: 16 rounds
-        xs.xs_clause_placement(256, 2, 16)
+    with pytest.raises(xs.XsError):                     # sets of 64 on 8 slots: 32 rounds
+        xs.xs_clause_placement(256, 2, 8)
     with pytest.raises(xs.XsError):                     # cap-32 order: 17+ sets
         xs.xs_clause_placement(512, 2, 32, xs.XS_FLAG_GAUGE, 32)
     with pytest.raises(xs.XsError):                     # odd slot count

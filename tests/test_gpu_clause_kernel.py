@@ -116,6 +116,7 @@ def test_clause_kernel_multi_instance_stop_rule_and_flip_table_switch():
     (100, 8, 1, True, 25, 128, 4),      # 4 sets of 25 on 32 slots
     (200, 8, 2, True, 50, 256, 4),      # 4 sets of 50 on 64 slots
     (96, 8, 1, False, 0, 128, 8),
+    (256, 8, 2, False, 32, 128, 11),    # the paper's cap-32 sets (L279): 9 and 11 rounds -> the long-list kernels
 ])
 def test_clause_kernel_ragged_orders_and_round_counts(N, W, I, balanced, cap, threads, rounds_max):
     """Orders that do not fill the CTA (idle slots on scratch rows), 5 / 7 / 8 rounds per sweep, sets
