@@ -329,7 +329,7 @@ def measure(name, wl, steps, warmup, ctx, with_e2e=True):
     return out
 
 
-def roofline_of(m, alu_peak, peaks):
+def roofline_of(m, alu_peak, peaks, sms=148):
     """The `roofline` object of a measured workload (dominant kernel = the sweep kernel)."""
     wl, lay, k_ms, ups, clocks = m["wl"], m["lay"], m["kernel_ms"], m["updates_per_step"], m["clocks"]
     N, W = wl["N"], wl["W"]
@@ -340,7 +340,7 @@ def roofline_of(m, alu_peak, peaks):
         roof = {"bound": "alu", "achieved": achieved, "peak": alu_peak / 1e3, "unit": "Tlop/s (32-bit LOP3/IADD lane-ops)",
                 "frac": achieved / (alu_peak / 1e3), "traffic": ncu.get("dram_bytes_per_launch"),
                 "peak_source": "xs_alu_peak LOP3 micro-kernel measured in this run",
-                "peak_nominal_at_sampled_clock": (148 * 64 * clocks["sm_mhz"] / 1e6) if clocks.get("sm_mhz") else None,
+                "peak_nominal_at_sampled_clock": (sms * 64 * clocks["sm_mhz"] / 1e6) if clocks.get("sm_mhz") else None,
                 "alg_ops_per_update": ALU_OPS_PER_UPDATE,
                 "alg_ops_model": "SURVEY.md 8(d): 14 lane-ops per 32 updates (algorithmic model, not pipe occupancy)",
                 "kernel": kname, "kernel_ms": k_ms}
@@ -362,7 +362,7 @@ def roofline_of(m, alu_peak, peaks):
         n_copies = 16 // lay.tile_words if lay.tile_words <= 16 else 1
         sm_bpu = {1: (6 + n_copies) * 16 / 128.0, 2: 6 * 16 / 128.0}.get(lay.variant, 11 * 16 / 128.0)
         if clocks.get("sm_mhz") and lay.variant != 3:
-            sm_peak = 148 * 128 * clocks["sm_mhz"] / 1e3                          # GB/s
+            sm_peak = sms * 128 * clocks["sm_mhz"] / 1e3                          # GB/s
             roof["shared_memory"] = {"bytes_per_update": sm_bpu,
                                      "achieved_gbs": sm_bpu * ups / (k_ms * 1e6),
                                      "peak_gbs": sm_peak,
@@ -443,6 +443,7 @@ def main():
     except OSError:
         pass
 
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
     m = measure(args.workload, wl, args.steps, args.warmup, ctx)
     alu_peak, _ = xs.xs_alu_peak()
     out = None
@@ -461,7 +462,7 @@ def main():
             "e2e": {"value": m["e2e_value"], "unit": "clone-spin updates/ns", "h2d_bytes_per_step": m["h2d"],
                     "d2h_bytes_per_step": m["d2h"]},
             "gpu_launches": m["launches"],
-            "roofline": roofline_of(m, alu_peak, peaks),
+            "roofline": roofline_of(m, alu_peak, peaks, sms),
             "energy": {"mean_per_spin": float(e_np.mean() / N), "min": int(e_np.min()), "max": int(e_np.max()),
                        "histogram": energy_histogram(e_np)},
         }
@@ -478,7 +479,7 @@ def main():
                 wmap[name] = {"error": f"{type(ex).__name__}: {ex}"}
                 continue
             if rank == 0:
-                r2 = roofline_of(m2, alu_peak, peaks)
+                r2 = roofline_of(m2, alu_peak, peaks, sms)
                 l2 = m2["lay"]
                 ent = {"value": m2["value"], "e2e": m2["e2e_value"], "ms_per_step": m2["total_ms"] / m2["steps"],
                        "roofline": {k: r2[k] for k in ("bound", "frac", "frac_own", "achieved", "peak", "unit", "kernel",
