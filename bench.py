@@ -54,6 +54,11 @@ WORKLOADS = {
                                metropolis=True,
                                desc="configs[1] with the Metropolis table w0 = w1^3, w2 = w3 = 1 (L69) at w1 = 0.055: N=256, "
                                     "2^16 clones, 1000 sweeps per step, first hits looked for after every sweep (clause-word kernel, W0 form)"),
+    # SURVEY.md 8(f) NEXT-2 on chip: per-clone noise on the config-2 workload (clause-word kernel, PCN form)
+    "config2_clone_noise": dict(N=256, W=1024, I=1, sweeps=500, graph_seed=2, run_seed=2, balanced=True, set_cap=64,
+                                clone_noise=True,
+                                desc="configs[1] with per-clone noise (XS_FLAG_CLONE_NOISE, w1 = 7/128): N=256, 2^16 clones, "
+                                     "500 sweeps per step (clause-word kernel, 16 x the Philox work)"),
     "config1": dict(N=64, W=1, I=1, sweeps=10_000, graph_seed=1, run_seed=1,
                     desc="configs[0] shape: N=64, 1 instance (graph seed 1), 64 clones, 10^4 sweeps per step, no early stop "
                          "(latency: one warp of work)"),
@@ -80,7 +85,7 @@ for _n, _s in ((128, 2000), (192, 1500), (256, 1000), (384, 700), (512, 500), (7
                                       desc=f"configs[3] shape: N={_n}, 128 instances, 2^14 clones each, {_s} sweeps "
                                            f"per step; update order = balanced independent sets (DESIGN.md R-balance)")
 # what the default run measures after the headline (short runs)
-EXTRAS = ["config1", "config2_greedy", "config2_cap32", "config2_metropolis", "config3", "config3_greedy"] + \
+EXTRAS = ["config1", "config2_greedy", "config2_cap32", "config2_metropolis", "config2_clone_noise", "config3", "config3_greedy"] + \
          [f"config4_{n}" for n in (128, 192, 256, 384, 512, 768, 1024)] + ["config5", "config5b"]
 
 # Integer-pipe work per update.

@@ -66,8 +66,9 @@ extern "C" {
                                     bit b, U = 7-bit number whose bit k is bit b of r_k, r_2j = o0|o1<<32,
                                     r_2j+1 = o2|o3<<32 of Philox(ctr=(i,4w+j,t,6), key=run seed), j=0..3;
                                     a k = 1 spin flips iff U < m, m = round(w1_threshold / 2^25)
-                                    (default: 7, w1 = 7/128).  Runs in the streaming regime; only the
-                                    quasi-greedy form of the flip table is accepted                    */
+                                    (default: 7, w1 = 7/128).  Runs on the clause-word kernel when the
+                                    batch has balanced sets that fill the CTA, else in the streaming
+                                    regime; only the quasi-greedy form of the flip table is accepted   */
 
 /* w1 = 0.055 (L101) as a 32-bit threshold: flip a k=1 spin iff u32 < floor(0.055 * 2^32). */
 #define XS_W1_THRESHOLD_DEFAULT 236223201u

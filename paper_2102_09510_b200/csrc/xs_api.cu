@@ -63,6 +63,23 @@ DevLayout make_layout(const xs_params& p)
 
 using namespace xs;
 
+// Launch geometry of a batch: the rule (choose_geometry), then the kernels with host-built tables
+// (clause-word, latency).  Per-clone noise exists on the clause-word kernel (full lists) and on the
+// streaming kernel only: a batch that the clause-word kernel does not take streams.
+static int settle_geometry(xs_batch* b, void* stream)
+{
+    std::string err;
+    b->p.flags = b->flags0;
+    if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
+    if (int e = clause_prepare(*b, stream)) return cuda_fail(e, "clause tables");
+    if (int e = warp_prepare(*b, stream)) return cuda_fail(e, "latency kernel tables");
+    if (b->ft.per_clone && b->geom.regime == 0 && b->geom.variant != 2) {
+        b->p.flags |= XS_FLAG_STREAMING;
+        if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
+    }
+    return XS_OK;
+}
+
 extern "C" {
 
 const char* xs_last_error(void) { return g_err.c_str(); }
@@ -152,15 +169,12 @@ static int finish_create(xs_batch* b, void* dev_ws, size_t ws_bytes, void* strea
     // quasi-greedy table (0, w1, 1, 1) of L67 / L101 until xs_set_flip_table says otherwise
     b->ft = FlipTable{{0u, p.w1_threshold, 0u, 0u}, 0xCu, 0u, 0u, 0u};
     if (p.flags & XS_FLAG_CLONE_NOISE) {
-        // per-clone noise: w1 = m / 128 with m the nearest integer; runs in the streaming regime
+        // per-clone noise: w1 = m / 128 with m the nearest integer
         b->ft.per_clone = 1u;
         b->ft.clone_m = (uint32_t)(((uint64_t)p.w1_threshold + (1ull << 24)) >> 25);
-        b->p.flags |= XS_FLAG_STREAMING;
     }
-    std::string err;
-    if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
-    if (int e = clause_prepare(*b, stream)) return cuda_fail(e, "clause tables");
-    if (int e = warp_prepare(*b, stream)) return cuda_fail(e, "latency kernel tables");
+    b->flags0 = b->p.flags;
+    if (int rc = settle_geometry(b, stream)) return rc;
     if (int e = launch_init(*b, stream)) return cuda_fail(e, "init kernel");
     if (int e = launch_mark(*b, true, stream)) return cuda_fail(e, "mark kernel");
     if (int e = launch_finalize(*b, 0, stream)) return cuda_fail(e, "finalize kernel");
@@ -264,11 +278,7 @@ int xs_set_flip_table(xs_batch* b, const uint64_t* thr4, void* cuda_stream)
     }
     b->ft = ft;
     if (!ft.general) b->p.w1_threshold = ft.lo[1];
-    std::string err;
-    if (!choose_geometry(*b, b->geom, err)) return fail(XS_EINVAL, err);
-    if (int e = clause_prepare(*b, cuda_stream)) return cuda_fail(e, "clause tables");
-    if (int e = warp_prepare(*b, cuda_stream)) return cuda_fail(e, "latency kernel tables");
-    return XS_OK;
+    return settle_geometry(b, cuda_stream);
 }
 
 int xs_set_geometry(xs_batch* b, const xs_geometry* g, void* cuda_stream)
@@ -285,14 +295,11 @@ int xs_set_geometry(xs_batch* b, const xs_geometry* g, void* cuda_stream)
     }
     const xs_geometry old = b->req;
     b->req = rq;
-    std::string err;
-    if (!choose_geometry(*b, b->geom, err)) {
+    if (int rc = settle_geometry(b, cuda_stream)) {
         b->req = old;
-        choose_geometry(*b, b->geom, err);
-        return fail(XS_EINVAL, err);
+        settle_geometry(b, cuda_stream);
+        return rc;
     }
-    if (int e = clause_prepare(*b, cuda_stream)) return cuda_fail(e, "clause tables");
-    if (int e = warp_prepare(*b, cuda_stream)) return cuda_fail(e, "latency kernel tables");
     return XS_OK;
 }
 

@@ -132,6 +132,7 @@ struct xs_batch {
     xs_geometry req{XS_GEOM_AUTO, 0, 0, 0, 0, 0};   // xs_set_geometry requests (0 / AUTO = rule)
     uint32_t num_sms = 148;       // cudaDevAttrMultiProcessorCount of the device the batch lives on
     int device = 0;               // CUDA device ordinal the workspace belongs to
+    uint32_t flags0 = 0;          // p.flags as given by the caller (p.flags may gain XS_FLAG_STREAMING)
     void* ws = nullptr;
 };
 

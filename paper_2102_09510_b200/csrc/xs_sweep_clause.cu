@@ -216,11 +216,12 @@ int clause_prepare(xs_batch& b, void* stream)
     TileGeom& g = b.geom;
     const xs_geometry& rq = b.req;
     if (rq.variant != XS_GEOM_AUTO && rq.variant != 2u) return 0;   // another kernel was asked for
-    if (g.regime != 0 || b.ft.per_clone || (b.p.flags & XS_FLAG_STREAMING)) return 0;
+    if (g.regime != 0 || (b.p.flags & XS_FLAG_STREAMING)) return 0;
     // flip tables: the quasi-greedy form (0, w1, 1, 1) and, on full lists (MODE 1), the family
     // (w0, w1, 1, 1) with 0 < w0 <= w1 (L69: Metropolis w0 = w1^3); anything else: generic kernel
     const bool family = b.ft.general && b.ft.always == 0xCu && b.ft.lo[0] > 0u && b.ft.lo[0] <= b.ft.lo[1];
     if (b.ft.general && !family) return 0;
+    const bool special = family || b.ft.per_clone;     // forms that exist for the full 4-8 round lists only
     if (rq.tile_words && rq.tile_words != CL_T) return 0;
     const uint32_t N = b.p.n_spins, I = b.p.n_instances, W = b.p.n_words;
     if (W % CL_T || N < 64u || N >= (1u << 14)) return 0;
@@ -275,7 +276,7 @@ int clause_prepare(xs_batch& b, void* stream)
         b.clause_rounds = rounds;
         b.clause_mode = mode == 3 ? 0u : mode;
     }
-    if (family && (b.clause_mode != 1u || rounds > CL_RCAP)) return 0;      // w0 > 0 needs the full lists
+    if (special && (b.clause_mode != 1u || rounds > CL_RCAP)) return 0;     // w0 > 0 / per-clone noise: full lists
     if (b.clause_thr != (uint64_t)b.p.w1_threshold) {
         // compare constants of the noise (xs_sweep_clause.cuh): 2^32 - thr, and the forced carry for thr = 0
         const uint32_t h[2] = {0u - b.p.w1_threshold, b.p.w1_threshold == 0u ? 1u : 0u};
@@ -315,6 +316,8 @@ int launch_sweep_clause(const xs_batch& b, uint32_t n_sweeps, void* stream)
     ClauseLaunch L;
     L.threads = g.threads; L.smem = g.smem; L.mode = b.clause_mode;
     L.w0 = b.ft.general != 0u;
+    L.pcn = b.ft.per_clone != 0u;
+    A.clone_m = b.ft.clone_m;
     L.dense = g.ctas > b.num_sms;
     L.st = (cudaStream_t)stream;
     const uint32_t tiles = b.p.n_words / CL_T;

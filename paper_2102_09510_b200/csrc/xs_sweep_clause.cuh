@@ -64,6 +64,7 @@ struct ClauseArgs {
     uint32_t off_misc;       // byte offset of det32 / known32 / flag in dynamic shared memory
     uint32_t thr;            // noise threshold: a k = 1 spin flips iff u < thr
     uint32_t thr0;           // W0 kernels: a k = 0 spin flips iff u < thr0 (thr0 <= thr)
+    uint32_t clone_m;        // PCN kernels: a k = 1 spin flips iff its clone's 7-bit number U < clone_m
     uint32_t one;            // the multiplier 1, as data, so that the compare stays a multiply-add
     uint32_t zero;           // the multiplier 0, as data: ties the last store of a round to its Philox call
     uint64_t seed[CL_MAXI];  // run seeds of instances inst0 .. (constant bank -> uniform registers)
@@ -109,7 +110,11 @@ constexpr int LUT_OR_ANDN = 0xF4;   // a | (b & ~c)
 //     threshold bit per word is kept (flip = M | (P & u<thr) | u<thr0), and a ground state can be
 //     left again: the first hit is looked for after EVERY sweep, without extra loads, by OR-ing
 //     every clause word at its LAST touch of the sweep (a static 3-bit mask per task, from the host).
-template <int R, int MAXTHREADS, int MINB, int MODE, bool W0 = false>
+// PCN: per-clone noise (XS_FLAG_CLONE_NOISE; DESIGN.md R-clone), MODE 1 only: every
+//     clone draws its own 7-bit number U from four Philox calls per (spin, word, sweep); a k = 1 spin
+//     flips iff U < clone_m.  Each lane computes the masks of its two words in the round itself (16 times
+//     the Philox work of the shared-number rule: this form is ALU bound).
+template <int R, int MAXTHREADS, int MINB, int MODE, bool W0 = false, bool PCN = false>
 __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_constant__ ClauseArgs A)
 {
     // One CTA per SM with few warps (fewer tiles than SMs, e.g. BASELINE.json configs[1]): the
@@ -275,6 +280,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     };
     // threshold bytes of the periods that contain sweep t
     auto produce_all = [&](uint32_t t) {
+        if (PCN) return;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             uint32_t own;
@@ -308,7 +314,26 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
                 // of the round and issues it first, interleaved with the update, in the shadow of
                 // the loads, instead of leaving the loads' latency exposed and the chain for later.
                 uint32_t a2 = ca[r][2];
-                if (hp == 1) {
+                uint32_t rc[CL_H] = {0u, 0u, 0u, 0u};     // PCN: k = 1 flip masks of the lane's four half words
+                if (PCN) {
+#pragma unroll
+                    for (int cw = 0; cw < 2; ++cw) {
+                        uint32_t rl[8], rh[8];            // low / high halves of r_0 .. r_7 of word w0 + 2 j + cw
+#pragma unroll
+                        for (int jj = 0; jj < 4; ++jj) {
+                            uint32_t q4[4];
+                            philox4x32_10(spin_of(r), 4u * (w0 + 2u * j + (uint32_t)cw) + (uint32_t)jj, t, TAG_CLONE,
+                                          k0, k1, q4);
+                            rl[2 * jj] = q4[0]; rh[2 * jj] = q4[1];
+                            rl[2 * jj + 1] = q4[2]; rh[2 * jj + 1] = q4[3];
+                        }
+                        const uint32_t lo7[7] = {rl[0], rl[1], rl[2], rl[3], rl[4], rl[5], rl[6]};
+                        const uint32_t hi7[7] = {rh[0], rh[1], rh[2], rh[3], rh[4], rh[5], rh[6]};
+                        rc[2 * cw] = clone_noise_mask(lo7, A.clone_m);
+                        rc[2 * cw + 1] = clone_noise_mask(hi7, A.clone_m);
+                    }
+                }
+                if (!PCN && hp == 1) {
                     uint32_t own;
                     rm[r] = noise_call(r, ((t + (uint32_t)(r & 1)) >> 1) + 1u, own);
                     if (!SPARSE) a2 = cl_mad_lo(own, A.zero, a2);
@@ -317,7 +342,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
                 for (int c = 0; c < CL_H; ++c) {
                     const uint32_t M = lop3<LUT_MAJ>(c0[c], c1[c], c2[c]);     // k >= 2
                     const uint32_t P = lop3<LUT_XOR3>(c0[c], c1[c], c2[c]);    // k odd
-                    uint32_t f = lop3<LUT_OR_ANDN>(M, P, nf[c >> 1]);          // flip mask (a-7)
+                    uint32_t f = PCN ? lop3<0xF8>(M, P, rc[c])                 // M | (P & R_clone)
+                                     : lop3<LUT_OR_ANDN>(M, P, nf[c >> 1]);    // flip mask (a-7)
                     if (W0) f = lop3<0xF3>(f, n0[c >> 1], 0u);                 // | (u < thr0): the k = 0 move
                     c0[c] ^= f; c1[c] ^= f; c2[c] ^= f;
                     x[r][c] ^= f;
@@ -456,23 +482,25 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
 struct ClauseLaunch {
     uint32_t threads, ctas, smem, mode;
     bool w0;             // flip table with w0 > 0 (MODE 1 only)
+    bool pcn;            // per-clone noise (MODE 1 only)
     bool dense;          // more CTAs than SMs: prefer the register-capped variants
     cudaStream_t st;
 };
 
-template <int R, int MT, int MINB, int MODE, bool W0 = false>
+template <int R, int MT, int MINB, int MODE, bool W0 = false, bool PCN = false>
 cudaError_t launch_clause_k(const ClauseArgs& A, const ClauseLaunch& L)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_clause<R, MT, MINB, MODE, W0>,
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_clause<R, MT, MINB, MODE, W0, PCN>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem);
     if (e != cudaSuccess) return e;
-    k_sweep_clause<R, MT, MINB, MODE, W0><<<L.ctas, L.threads, L.smem, L.st>>>(A);
+    k_sweep_clause<R, MT, MINB, MODE, W0, PCN><<<L.ctas, L.threads, L.smem, L.st>>>(A);
     return cudaGetLastError();
 }
 
 template <int R, int MT, int MINB>
 cudaError_t launch_clause_m(const ClauseArgs& A, const ClauseLaunch& L)
 {
+    if (L.mode == 1 && L.pcn) return launch_clause_k<R, MT, MINB, 1, false, true>(A, L);
     if (L.mode == 1 && L.w0) return launch_clause_k<R, MT, MINB, 1, true>(A, L);
     if (L.mode == 1) return launch_clause_k<R, MT, MINB, 1>(A, L);
     if (L.mode == 2 && R % 2 == 0) return launch_clause_k<R, MT, MINB, (R % 2 == 0 ? 2 : 0)>(A, L);

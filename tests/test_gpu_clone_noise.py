@@ -63,3 +63,31 @@ def test_clone_noise_multi_instance_stop_rule_and_first_hits():
         _compare(b, oracles, "clone noise stop rule")
     assert any(o.solved for o in oracles)
     b.close()
+
+
+@pytest.mark.parametrize("N,W,I,m", [(128, 8, 2, None), (256, 16, 1, None), (192, 8, 1, 40), (512, 8, 1, 1), (384, 8, 1, None)])
+def test_clone_noise_on_the_clause_word_kernel(N, W, I, m):
+    """SURVEY.md 8(f) NEXT-2 on chip: with balanced sets that fill the CTA (4 - 8 rounds) the per-clone
+    noise runs on the clause-word kernel (layout regime 0, variant 2), each lane drawing the 7-bit
+    numbers of its two words' 128 clones from 8 Philox calls per round."""
+    import paper_2102_09510_b200 as xs
+    fl = xs.XS_FLAG_GAUGE | xs.XS_FLAG_NO_SKIP | xs.XS_FLAG_CLONE_NOISE | xs.XS_FLAG_BALANCED
+    gs, rs = [N + 60 + i for i in range(I)], [4 * N + i for i in range(I)]
+    b = xs.Batch(N, W, gs, rs, flags=fl, geometry=dict(batch_sweeps=16))
+    if m is not None:
+        b.set_flip_table([0, m << 25, 1 << 32, 1 << 32])
+    lay = b.layout()
+    assert (lay.regime, lay.variant, lay.tile_words) == (0, 2, 8), (lay.regime, lay.variant)
+    os_ = [OracleRun(N, W, g, r, no_skip=True, balanced=True, clone_m=7 if m is None else m) for g, r in zip(gs, rs)]
+    for n in (1, 2, 19):
+        b.run_sweeps(n)
+        for o in os_:
+            o.run_sweeps(n)
+    _compare(b, os_, f"clone noise on chip N={N} W={W}")
+    b.set_geometry(variant=0)                      # no other on-chip kernel has it: the batch streams
+    assert b.layout().regime == 1
+    b.run_sweeps(5)
+    for o in os_:
+        o.run_sweeps(5)
+    _compare(b, os_, "clone noise, back to streaming")
+    b.close()
