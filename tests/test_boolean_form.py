@@ -70,7 +70,16 @@ def test_clause_word_forms_equal_pm1_rule_on_all_inputs():
     or_andn = int(m.group(1), 16)
     assert re.search(r"M = lop3<LUT_MAJ>\(c0\[c\], c1\[c\], c2\[c\]\)", cl)
     assert re.search(r"P = lop3<LUT_XOR3>\(c0\[c\], c1\[c\], c2\[c\]\)", cl)
-    assert re.search(r"f = lop3<LUT_OR_ANDN>\(M, P, nf\[c >> 1\]\)", cl)      # nf = NOT-flip mask (u >= thr)
+    assert re.search(r"lop3<LUT_OR_ANDN>\(M, P, nf\[c >> 1\]\)", cl)          # nf = NOT-flip mask (u >= thr)
+    m = re.search(r"f = PCN \? lop3<(0x[0-9A-Fa-f]+)>\(M, P, rc\[c\]\)", cl)     # per-clone noise: rc = flip mask
+    assert m
+    pcn_lut = int(m.group(1), 16)
+    m = re.search(r"if \(W0\) f = lop3<(0x[0-9A-Fa-f]+)>\(f, n0\[c >> 1\], 0u\);", cl)   # n0 = NOT-flip mask of k = 0
+    assert m
+    w0_lut = int(m.group(1), 16)
+    m = re.search(r"lacc\[c\] = lop3<(0x[0-9A-Fa-f]+)>\(c0\[c\], l0, lacc\[c\]\);", cl)
+    assert m
+    acc_lut = int(m.group(1), 16)
     assert re.search(r"c0\[c\] \^= f; c1\[c\] \^= f; c2\[c\] \^= f;\s*x\[r\]\[c\] \^= f;", cl)
     m = re.search(r"PACK \? lop3<(0x[0-9A-Fa-f]+)>\(nb, rm\[r\], 0x80808080u\) : nb", cl)
     assert m
@@ -92,12 +101,19 @@ def test_clause_word_forms_equal_pm1_rule_on_all_inputs():
         # clause-word kernel: threshold bytes hold NOT R
         M, P = lop3(L["LUT_MAJ"], *c), lop3(L["LUT_XOR3"], *c)
         assert lop3(or_andn, M, P, 1 - R) == flip, bits
+        assert lop3(pcn_lut, M, P, R) == flip, bits
+        # tables (w0, w1, 1, 1), w0 <= w1, one number per word: R0 = (u < thr0) implies R = (u < thr1)
+        for R0 in ((0, 1) if R else (0,)):
+            flip_w0 = int((k >= 2) or (k == 1 and R == 1) or (k == 0 and R0 == 1))
+            assert lop3(w0_lut, lop3(or_andn, M, P, 1 - R), 1 - R0, 0) == flip_w0, bits
         # after the flip the clause bits must be those of the new spin value
         x_new = x ^ flip
         c_new = [x_new ^ a0 ^ b0 ^ j0, x_new ^ a1 ^ b1 ^ j1, x_new ^ a2 ^ b2 ^ j2]
         assert [ci ^ flip for ci in c] == c_new, bits
         # latency kernel: the same with the mask R itself
         assert lop3(or_and, M, P, R) == flip, bits
+    for a, b, cc in itertools.product((0, 1), repeat=3):
+        assert lop3(acc_lut, a, b, cc) == ((a & b) | cc)              # last-touch accumulate
     # the merge of new threshold bits into the register that also carries the spin index
     for a, b, cc in itertools.product((0, 1), repeat=3):
         assert lop3(merge, a, b, cc) == (a if cc else b)
