@@ -65,7 +65,8 @@ __device__ __forceinline__ void bar_arrive(uint32_t id, uint32_t count)
 
 // shared memory: [W][N + 16] uint64 clause words (+ one scratch word per slot), then the ring
 // [2][WP_KB][n_pass * 16][W] uint32 noise masks
-template <int RMAX>
+// NP: passes per sweep (exact: the pass loop carries no tests).
+template <int NP>
 __global__ void __launch_bounds__(32 * (4 + WP_PROD), 1) k_sweep_warp(WarpArgs A)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -118,19 +119,14 @@ __global__ void __launch_bounds__(32 * (4 + WP_PROD), 1) k_sweep_warp(WarpArgs A
     uint64_t* xg = A.d.x + (size_t)inst * N * W + w;
     uint32_t* fhg = A.d.first_hit + ((size_t)inst * W + w) * 64;
 
-    uint32_t ca[RMAX][3], spin[RMAX], x[RMAX];
+    uint32_t ca[NP][3], spin[NP], x[NP];
 #pragma unroll
-    for (int r = 0; r < RMAX; ++r) {
-        if (r < (int)A.n_pass) {
-            const CRec v = cr[r * WP_SLOTS + slot];
-            ca[r][0] = col + v.off0 + 4u * half;
-            ca[r][1] = col + v.off1 + 4u * half;
-            ca[r][2] = col + v.off2 + 4u * half;
-            spin[r] = v.spin;
-        } else {
-            ca[r][0] = ca[r][1] = ca[r][2] = col;
-            spin[r] = WP_IDLE;
-        }
+    for (int r = 0; r < NP; ++r) {
+        const CRec v = cr[r * WP_SLOTS + slot];
+        ca[r][0] = col + v.off0 + 4u * half;
+        ca[r][1] = col + v.off1 + 4u * half;
+        ca[r][2] = col + v.off2 + 4u * half;
+        spin[r] = v.spin;
         x[r] = 0;
     }
     auto load_state = [&]() {
@@ -143,14 +139,14 @@ __global__ void __launch_bounds__(32 * (4 + WP_PROD), 1) k_sweep_warp(WarpArgs A
             wp_sts(col + 8u * t + 4u, (uint32_t)(v >> 32));
         }
 #pragma unroll
-        for (int r = 0; r < RMAX; ++r)
+        for (int r = 0; r < NP; ++r)
             if (spin[r] != WP_IDLE)
                 x[r] = reinterpret_cast<const uint32_t*>(xg + (size_t)spin[r] * W)[half];
         __syncwarp();
     };
     auto store_state = [&]() {
 #pragma unroll
-        for (int r = 0; r < RMAX; ++r)
+        for (int r = 0; r < NP; ++r)
             if (spin[r] != WP_IDLE)
                 reinterpret_cast<uint32_t*>(xg + (size_t)spin[r] * W)[half] = x[r];
     };
@@ -175,8 +171,8 @@ __global__ void __launch_bounds__(32 * (4 + WP_PROD), 1) k_sweep_warp(WarpArgs A
     // one sweep with the noise of slot `kb` of buffer `nbase`
     auto sweep = [&](uint32_t nrow) {
 #pragma unroll
-        for (int r = 0; r < RMAX; ++r) {
-            if (r < (int)A.n_pass) {
+        for (int r = 0; r < NP; ++r) {
+            {
                 const uint32_t c0 = wp_lds(ca[r][0]), c1 = wp_lds(ca[r][1]), c2 = wp_lds(ca[r][2]);
                 const uint32_t R = wp_lds(nrow + ((uint32_t)r * WP_SLOTS + slot) * W * 4u);
                 const uint32_t M = lop3<LUT_MAJ>(c0, c1, c2);       // k >= 2
@@ -299,16 +295,20 @@ int launch_sweep_warp(const xs_batch& b, uint32_t n_sweeps, void* stream)
     A.ent = crec_entries(b.p);
     A.off_ring = A.W * warp_col_bytes(A.N);
     cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e;
-    if (A.n_pass <= 8) {
-        e = cudaFuncSetAttribute(k_sweep_warp<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
-        if (e != cudaSuccess) return (int)e;
-        k_sweep_warp<8><<<g.ctas, g.threads, g.smem, st>>>(A);
-    } else {
-        e = cudaFuncSetAttribute(k_sweep_warp<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
-        if (e != cudaSuccess) return (int)e;
-        k_sweep_warp<16><<<g.ctas, g.threads, g.smem, st>>>(A);
+    cudaError_t e = cudaErrorInvalidValue;
+#define XS_WP_CASE(NP_)                                                                                        \
+    case NP_:                                                                                                  \
+        e = cudaFuncSetAttribute(k_sweep_warp<NP_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem); \
+        if (e != cudaSuccess) return (int)e;                                                                   \
+        k_sweep_warp<NP_><<<g.ctas, g.threads, g.smem, st>>>(A);                                               \
+        break;
+    switch (A.n_pass) {
+        XS_WP_CASE(1) XS_WP_CASE(2) XS_WP_CASE(3) XS_WP_CASE(4) XS_WP_CASE(5) XS_WP_CASE(6) XS_WP_CASE(7) XS_WP_CASE(8)
+        XS_WP_CASE(9) XS_WP_CASE(10) XS_WP_CASE(11) XS_WP_CASE(12) XS_WP_CASE(13) XS_WP_CASE(14) XS_WP_CASE(15)
+        XS_WP_CASE(16)
+        default: return (int)cudaErrorInvalidValue;
     }
+#undef XS_WP_CASE
     e = cudaGetLastError();
     if (e != cudaSuccess) return (int)e;
     count_launch(1);
