@@ -156,8 +156,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     // spills under the 128-register cap.  (Measured: the unpacking costs 6 % with 4 rounds, where
     // there is room, and gains 3 % with 8.)
     constexpr bool PACK = (R >= 7);
-    uint32_t rm[R];
-    uint32_t spin[PACK ? 1 : R];
+    uint32_t rm[R] = {};
+    uint32_t spin[PACK ? 1 : R] = {};
     auto spin_of = [&](int r) -> uint32_t {
         return PACK ? ((rm[r] & 0x7Fu) | ((rm[r] >> 1) & 0x3F80u)) : spin[PACK ? 0 : r];
     };
@@ -280,11 +280,12 @@ __global__ void __launch_bounds__(MAXTHREADS, MINB) k_sweep_clause(const __grid_
     };
     // threshold bytes of the periods that contain sweep t
     auto produce_all = [&](uint32_t t) {
-        if (PCN) return;
+        if (!PCN) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            uint32_t own;
-            rm[r] = noise_call(r, (t + (uint32_t)(r & 1)) >> 1, own);
+            for (int r = 0; r < R; ++r) {
+                uint32_t own;
+                rm[r] = noise_call(r, (t + (uint32_t)(r & 1)) >> 1, own);
+            }
         }
     };
 
