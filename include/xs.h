@@ -24,6 +24,9 @@
  *     E = -N (0 if the initial state already has; XS_NO_HIT = never so far).
  *   - Every call returns 0 (XS_OK) or a negative error code; nothing throws or aborts across
  *     the ABI; xs_last_error() returns a thread-local description of the last failure.
+ *   - A batch lives on the CUDA device that is current when it is created; every later call on it
+ *     must be made with that device current and a stream of that device (the Python binding's
+ *     Batch does this for the caller).
  *   - All calls that take a stream only enqueue work on it; xs_tts also synchronises it.
  *     xs_create_instance* additionally block the host until the table uploads are done.
  */
@@ -102,7 +105,8 @@ typedef struct {
     uint32_t batch_sweeps;   /* sweeps between ground-state checks inside the kernel             */
     uint32_t n_sets_max;     /* largest number of independent sets over the instances            */
     uint32_t variant;        /* on-chip: 0 = generic tile kernel, 1 = static-task (spin-word)
-                                kernel, 2 = clause-word kernel, 3 = single-warp latency kernel  */
+                                kernel, 2 = clause-word kernel, 3 = latency kernel (W <= 4 words:
+                                one consumer warp per word + noise producer warps)               */
 } xs_layout;
 
 /* Explicit launch geometry (xs_set_geometry).  Every field is a request: 0 (XS_GEOM_AUTO for
