@@ -257,6 +257,20 @@ int xs_tts_stats(const uint32_t* tts, uint32_t n_runs, uint64_t t_max, double* o
  * Returns XS_EINVAL for K < 3 or T <= 0. */
 int xs_cavity_barrier(uint32_t K, double T, double* out /* [6] */);
 
+/* Allocation-free ground-state check, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it).  dev_mask [n_instances][n_words] uint64
+ * (device, caller-owned): bit b of word w is set iff clone 64 w + b of that instance is in a ground
+ * state NOW, i.e. has no unsatisfied interaction, E = -N (the between-launch check of
+ * L71) -- the same clones for which xs_energy gives -n_spins.  Asynchronous on cuda_stream.
+ * The scratch of the detection kernel (one uint64 per (instance, word)) lives in a static device
+ * array inside the library, XS_STATIC_MAX_WORDS words = 512 KiB that every GPU which loads the library
+ * holds until exit; the call performs no cudaMalloc / cudaFree and calls no allocating routine.
+ * XS_EINVAL if n_instances * n_words > XS_STATIC_MAX_WORDS; XS_ESTATE if the batch's device is not
+ * current.  All calls (of all batches, on one GPU) share the array: each clears the part it uses,
+ * and calls that OVERLAP on the GPU (different streams without a dependency) race -- serialise them. */
+#define XS_STATIC_MAX_WORDS 65536
+int xs_solved_mask_static(xs_batch* b, uint64_t* dev_mask /* [inst][W] */, void* cuda_stream);
+
 /* Measurement helpers (no arithmetic of the method).
  * xs_alu_peak: runs a pure-LOP3 micro-kernel (16 independent chains per thread, all SMs) and
  *   returns the measured integer-pipe rate in 32-bit lane-operations per nanosecond for the

@@ -13,7 +13,7 @@ from ._binding import (XS_FLAG_BALANCED, XS_FLAG_CLONE_NOISE, XS_FLAG_GAUGE, XS_
                        xs_create_instance, xs_kernel_launches,
                        xs_create_instance_from_arrays, xs_destroy, xs_energy, xs_get_first_hit,
                        xs_clause_placement, xs_generate_graph, xs_get_graph, xs_get_layout, xs_get_spins, xs_params, xs_run_sweeps, xs_set_flip_table, xs_set_geometry, XS_GEOM_AUTO,
-                       xs_set_spins, xs_tts, xs_tts_rec, xs_tts_stats, xs_workspace_bytes)
+                       xs_set_spins, xs_solved_mask_static, XS_STATIC_MAX_WORDS, xs_tts, xs_tts_rec, xs_tts_stats, xs_workspace_bytes)
 
 
 class Batch:
@@ -100,6 +100,16 @@ class Batch:
         with self._on():
             out = torch.empty((self.n_instances, 64 * self.W), dtype=torch.int32, device=self.device)
             xs_get_first_hit(self.h, out.data_ptr(), stream)
+        return out
+
+    def solved_mask_static(self, out=None, stream=None):
+        """xs_solved_mask_static into `out` (int64 [instances][W], caller-owned; allocated here if None)."""
+        import torch
+        with self._on():
+            if out is None:
+                out = torch.empty((self.n_instances, self.W), dtype=torch.int64, device=self.device)
+            assert out.is_cuda and out.is_contiguous() and out.numel() == self.n_instances * self.W
+            xs_solved_mask_static(self.h, out.data_ptr(), stream)
         return out
 
     def get_graph(self, inst: int = 0):

@@ -45,7 +45,7 @@ XS_GEOM_AUTO = 0xFFFFFFFF
 EXPORTS = ["xs_workspace_bytes", "xs_create_instance", "xs_create_instance_from_arrays",
            "xs_run_sweeps", "xs_set_flip_table", "xs_set_geometry", "xs_energy", "xs_tts", "xs_get_spins", "xs_set_spins",
            "xs_get_first_hit", "xs_get_graph", "xs_generate_graph", "xs_clause_placement", "xs_get_layout", "xs_tts_stats",
-           "xs_cavity_barrier", "xs_alu_peak", "xs_kernel_launches", "xs_destroy",
+           "xs_cavity_barrier", "xs_alu_peak", "xs_kernel_launches", "xs_solved_mask_static", "xs_destroy",
            "xs_last_error"]
 
 _lib = None
@@ -81,6 +81,7 @@ def lib():
     L.xs_get_layout.argtypes = [vp, C.POINTER(xs_layout)]
     L.xs_tts_stats.argtypes = [u32p, C.c_uint32, C.c_uint64, C.POINTER(C.c_double)]
     L.xs_cavity_barrier.argtypes = [C.c_uint32, C.c_double, C.POINTER(C.c_double)]
+    L.xs_solved_mask_static.argtypes = [vp, vp, vp]
     L.xs_destroy.argtypes = [vp]
     L.xs_alu_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
     L.xs_kernel_launches.argtypes = []
@@ -269,6 +270,14 @@ def xs_alu_peak(stream=None):
     v, ms = C.c_double(0), C.c_double(0)
     _check(lib().xs_alu_peak(C.byref(v), C.byref(ms), _stream(stream)), "xs_alu_peak")
     return float(v.value), float(ms.value)
+
+
+XS_STATIC_MAX_WORDS = 65536
+
+
+def xs_solved_mask_static(h, dev_mask_ptr: int, stream=None):
+    """Allocation-free ground-state mask (include/xs.h): static scratch inside the library."""
+    _check(lib().xs_solved_mask_static(h, C.c_void_p(dev_mask_ptr), _stream(stream)), "xs_solved_mask_static")
 
 
 def xs_kernel_launches() -> int:

@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libxs_b200.so")
 OBJ = os.path.join(_HERE, "_obj")      # object cache (git-ignored); sources compile in parallel
-SOURCES = ["xs_api.cu", "xs_kernels.cu", "xs_sweep_static.cu", "xs_sweep_clause.cu", "xs_sweep_warp.cu", "xs_diag.cu", "xs_graph.cpp", "xs_stats.cpp"] + \
+SOURCES = ["xs_api.cu", "xs_kernels.cu", "xs_sweep_static.cu", "xs_sweep_clause.cu", "xs_sweep_warp.cu", "xs_static.cu", "xs_diag.cu", "xs_graph.cpp", "xs_stats.cpp"] + \
           [f"xs_sweep_static_i{cw}{nc}.cu" for cw in (1, 2) for nc in (1, 2, 4)] + \
           [f"xs_sweep_clause_r{r}.cu" for r in range(4, 17)]
 HEADERS = ["xs_internal.h", "xs_device.cuh", "xs_sweep_static.cuh", "xs_sweep_clause.cuh", os.path.join("..", "..", "include", "xs.h")]

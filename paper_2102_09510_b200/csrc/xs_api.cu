@@ -38,6 +38,8 @@ int check_params(const xs_params* p)
 }  // namespace
 
 namespace xs {
+int xs_set_error(int code, const std::string& msg) { return fail(code, msg); }
+
 DevLayout make_layout(const xs_params& p)
 {
     DevLayout L;

@@ -137,6 +137,8 @@ struct xs_batch {
 };
 
 namespace xs {
+// sets the thread-local message behind xs_last_error() and returns `code` (xs_api.cu)
+int xs_set_error(int code, const std::string& msg);
 // kernels (xs_kernels.cu); every launcher returns a cudaError_t as int.
 int launch_init(const xs_batch& b, void* stream);
 int launch_mark(const xs_batch& b, bool reset_first_hit, void* stream);   // ground-state marking at current t
